@@ -1,0 +1,26 @@
+"""Build oracle/libic_oracle.so with gcc.  TEST INFRASTRUCTURE (see ic_oracle.c).
+
+-ffp-contract=off: the oracle's floating point is plain IEEE fp64, one rounding
+per operation (reading U2).
+"""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SOURCES = ["ic_oracle.c", "ic_enum.c"]
+LIB = os.path.join(HERE, "libic_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    srcs = [os.path.join(HERE, s) for s in SOURCES]
+    deps = srcs + [os.path.join(HERE, "ic_oracle.h")]
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+        return LIB
+    cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+           "-Wall", "-Wextra", "-o", LIB] + srcs + ["-lm"]
+    subprocess.run(cmd, check=True, cwd=HERE)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))
