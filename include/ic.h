@@ -1,0 +1,135 @@
+/*
+ * include/ic.h -- C ABI of the B200 coupled-pair Metropolis library (libic_b200.so).
+ *
+ * Hot path of arXiv:2301.11735 (Budrin, Ulitko, Chikov, Panov, Moskvin): the charge-conserving parallel
+ * Metropolis sweep with "coupled pairs" (sec. 3.1) on an L x L periodic square lattice of
+ * 4-state sites, followed by the per-sweep reductions that feed C(T) and chi(T) (sec. 2.2).
+ * All arithmetic of the path runs in hand-written sm_100a CUDA kernels; the host side of the library only
+ * validates arguments, builds the acceptance-threshold tables and the O(1) schedule parameters, and launches.
+ *
+ * Conventions
+ *   - plain C, no exceptions; every entry point returns IC_OK (0) or a negative IC_ERR_* code and leaves
+ *     the context unchanged on error.  ic_strerror() gives the text (for IC_ERR_CUDA the CUDA message).
+ *   - pointers named h_* are HOST memory, d_* are DEVICE memory; both stay owned by the caller.  The
+ *     library never allocates device memory: everything it keeps on the device lives inside the
+ *     caller-provided workspace (a torch tensor in the Python binding).
+ *   - site code c (public, in ic_set_state / ic_state):   0 -> sigma=+1 (s=+1/2),  1 -> sigma=-1,
+ *     2 -> S=+1,  3 -> S=-1   (S=+-1 charge states, S=0 with s=+-1/2 magnetic states,
+ *     sigma = 2(1-S^2)s).  Lattices are row-major, code[y*L + x], periodic in x and y.
+ *   - exact integers of a lattice: n2 = sum S_i^2, bV = sum_<ij> S_i S_j, bJ = sum_<ij> sigma_i sigma_j
+ *     (each site contributes its +x and +y bond), so that eq. (3) reads
+ *     E = Delta*n2 + V*bV + (J/4)*bJ;  M = sum sigma_i, Ms = sum (-1)^(x+y) sigma_i, Q = sum S_i.
+ *   - the constraint of eq. (2), sum_i S_i = Q = llround(n*N), holds after every pair update.
+ *   - all launches and copies go to the CUDA stream given to ic_create.  ic_sweep is asynchronous;
+ *     ic_observables, ic_state, ic_debug_recompute and ic_thresholds synchronise that stream.
+ *   - one context must not be used from two host threads at once.
+ */
+#ifndef IC_H
+#define IC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ic_ctx ic_ctx; /* opaque; owned by the library from ic_create to ic_destroy */
+
+enum {
+  IC_OK = 0,
+  IC_ERR_NULL = -1,      /* a required pointer is NULL                                                */
+  IC_ERR_SIZE = -2,      /* L not a power of two or L < 4 or L > 65536, replicas < 1, bits not 8 or 2,
+                            replica index out of range                                                */
+  IC_ERR_PARAM = -3,     /* |n| > 1, NaN/inf parameter, T <= 0, nsweeps < 0, sweep counter >= 2^31     */
+  IC_ERR_WORKSPACE = -4, /* workspace NULL, smaller than ic_workspace_bytes(), or not 256-B aligned   */
+  IC_ERR_CHARGE = -5,    /* ic_set_state: a code outside 0..3 or sum S != Q; ic_init_charges: bad counts */
+  IC_ERR_CUDA = -6       /* a CUDA call failed; ic_strerror(IC_ERR_CUDA) returns its message          */
+};
+
+/* Filled by ic_observables, one per replica (host memory, caller-owned).
+ * C and chi follow PAPER.md:51 with k_B = 1:  C = (<E^2> - <E>^2) / (N T^2); the paper names chi(T)
+ * (Fig. 6) without a formula, reading G9: chi_u = (<M^2> - <M>^2) / (N T) and
+ * chi_s the same with Ms.  Averages are sums / nmeas. */
+typedef struct {
+  int64_t nmeas;                  /* sweeps accumulated since create / ic_reset_observables          */
+  int64_t n2, bV, bJ, M, Ms, Q;   /* exact integers of the current lattice                           */
+  double sumE, sumE2, sumM, sumM2, sumAbsM, sumMs, sumMs2, sumAbsMs; /* fp64, added once per sweep   */
+  double T, C, chi_u, chi_s;      /* derived with the T given to the last ic_sweep call (0 if none)  */
+} ic_obs;
+
+/* Number of acceptance classes per temperature: index = ((dn2/2+1)*33 + (dV+16))*33 + (dJ+16) with
+ * dn2 in {-2,0,2}, dV and dJ in [-16,16] (E_Delta, E_V, E_J of eq. 4/5).            */
+#define IC_N_CLASSES 3267
+
+/* Bytes of device memory ic_create needs for (L, replicas, bits_per_site); 0 if the arguments are invalid. */
+size_t ic_workspace_bytes(int L, int replicas, int bits_per_site);
+
+/* Creates a context for `replicas` independent copies of an L x L lattice (several copies
+ * processed in parallel) with parameters Delta, V, J of eq. (1)/(3), charge density n
+ * (eq. 2: Q = llround(n*L*L)) and Philox key `seed`.  Every replica r is initialised by stage 1
+ * (PAPER.md:59-62): random sigma on all sites, then |Q| distinct random sites set to S = sign(Q), drawn
+ * from the counter-based stream (seed, replica r) -- DESIGN.md "U0".  bits_per_site: 8 (one byte per site)
+ * or 2 (16 sites per 32-bit word) in device memory.
+ * d_workspace: device memory, >= ic_workspace_bytes() bytes, 256-B aligned, owned by the caller and kept
+ * alive until ic_destroy.  cuda_stream: a cudaStream_t (NULL = default stream).                      */
+int ic_create(ic_ctx** out, int L, double n, double delta, double V, double J, uint64_t seed, int replicas,
+              int bits_per_site, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Re-runs stage 1 for one replica with nplus sites S=+1 and nminus sites S=-1 (nplus - nminus must equal Q,
+ * nplus + nminus <= N); used for neutral lattices with charges of both signs (BASELINE config 3).    */
+int ic_init_charges(ic_ctx* ctx, int replica, int64_t nplus, int64_t nminus);
+
+/* Replaces the lattice of one replica by h_codes[L*L] (public codes, row-major, HOST memory) after checking
+ * every code and sum S == Q; recomputes the replica's exact integers on the device.                   */
+int ic_set_state(ic_ctx* ctx, int replica, const int8_t* h_codes);
+
+/* Runs nsweeps sweeps on all replicas, replica r at temperature h_T[r] (HOST array of `replicas` doubles,
+ * read before the call returns).  One sweep = N/2 coupled-pair updates in two conflict-free phases in which
+ * every site belongs to exactly one pair (schedule S1 of DESIGN.md; PAPER.md:108-125 requires only that
+ * concurrently updated pairs do not interact).  A pair update is PAPER.md:64-98: q = S_a + S_b, new pair
+ * configuration drawn from the table of configurations with the same q, dE from eq. (4)/(5), accepted with
+ * min(1, exp(-dE/T)) as an integer comparison with a host-built threshold.  After each sweep E, E^2, M, ...
+ * are accumulated.  The sweep counter is global: ic_sweep(T,100) == ic_sweep(T,50) twice.
+ * Asynchronous on the context's stream.                                                              */
+int ic_sweep(ic_ctx* ctx, const double* h_T, int64_t nsweeps);
+
+/* Same, and writes (n2,bV,bJ,M,Ms,Q) after every sweep to d_trace[s][r][6] (DEVICE memory, int64,
+ * nsweeps*replicas*6 entries, caller-owned).                                                         */
+int ic_sweep_trace(ic_ctx* ctx, const double* h_T, int64_t nsweeps, int64_t* d_trace);
+
+int ic_reset_observables(ic_ctx* ctx);            /* zeroes nmeas and the fp64 sums (not the lattice)  */
+int ic_observables(ic_ctx* ctx, ic_obs* h_out);   /* h_out[replicas], HOST; synchronises the stream    */
+int ic_state(ic_ctx* ctx, int replica, int8_t* h_codes_out); /* L*L public codes, HOST; synchronises   */
+
+/* Full recomputation of (n2,bV,bJ,M,Ms,Q) from the lattice by a device reduction, straight from eq. (3);
+ * out6 is HOST memory.  Must equal the incrementally tracked integers at any time.                    */
+int ic_debug_recompute(ic_ctx* ctx, int replica, int64_t* out6);
+
+/* The acceptance-threshold table the device uses for temperature T: h_out[IC_N_CLASSES] (HOST).  Entry
+ * t29 in [1, 2^29]: a move with 32-bit random word w is accepted iff (w >> 3) < t29, t29 = 2^29 for dE <= 0
+ * else clamp(floor(exp(-dE/T) * 2^29), 1, 2^29 - 1), dE = (Delta*dn2 + V*dV) + (J/4)*dJ in IEEE fp64. */
+int ic_thresholds(ic_ctx* ctx, double T, uint32_t* h_out);
+
+/* Schedule parameters of sweep `sweep` as the device will use them: out4 = {0, mx, my, 0} for a FAR sweep
+ * (partner(x,y) = (x^mx, y^my)), {1, orientation, offset, 0} for a NEAR sweep (dominoes).  HOST.      */
+int ic_schedule(ic_ctx* ctx, uint64_t sweep, int32_t* out4);
+
+int64_t ic_sweep_count(const ic_ctx* ctx);        /* global sweep counter; -1 if ctx is NULL           */
+int64_t ic_charge(const ic_ctx* ctx);             /* Q = llround(n*N); 0 if ctx is NULL                */
+
+/* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
+ * 2 = tiled kernels, 3 = shared-memory-resident multi-sweep kernel.  IC_ERR_PARAM if the variant cannot
+ * run this context's (L, bits_per_site).  All variants produce identical lattices.                   */
+int ic_set_variant(ic_ctx* ctx, int variant);
+
+/* Number of kernels launched by this context since ic_create (for bench.py's gpu_launches).         */
+int64_t ic_launch_count(const ic_ctx* ctx);
+
+int ic_destroy(ic_ctx* ctx);
+const char* ic_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IC_H */

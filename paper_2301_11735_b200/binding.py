@@ -1,0 +1,180 @@
+"""ctypes binding of libic_b200.so -- same names as include/ic.h, argument marshalling only.
+
+PyTorch is used for device memory (the workspace tensor, trace buffers) and the CUDA stream; every step of the
+path runs in the library's kernels.  There is no CPU fallback: if the library cannot be built or loaded, importing
+this module raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+IC_OK, IC_ERR_NULL, IC_ERR_SIZE, IC_ERR_PARAM, IC_ERR_WORKSPACE, IC_ERR_CHARGE, IC_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
+IC_N_CLASSES = 3267
+
+
+class ic_obs(C.Structure):
+    _fields_ = [("nmeas", C.c_int64), ("n2", C.c_int64), ("bV", C.c_int64), ("bJ", C.c_int64), ("M", C.c_int64),
+                ("Ms", C.c_int64), ("Q", C.c_int64),
+                ("sumE", C.c_double), ("sumE2", C.c_double), ("sumM", C.c_double), ("sumM2", C.c_double),
+                ("sumAbsM", C.c_double), ("sumMs", C.c_double), ("sumMs2", C.c_double), ("sumAbsMs", C.c_double),
+                ("T", C.c_double), ("C", C.c_double), ("chi_u", C.c_double), ("chi_s", C.c_double)]
+
+
+EXPORTS = {
+    "ic_workspace_bytes": (C.c_size_t, [C.c_int, C.c_int, C.c_int]),
+    "ic_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_uint64,
+                            C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "ic_init_charges": (C.c_int, [C.c_void_p, C.c_int, C.c_int64, C.c_int64]),
+    "ic_set_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "ic_sweep": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_int64]),
+    "ic_sweep_trace": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_int64, C.c_void_p]),
+    "ic_reset_observables": (C.c_int, [C.c_void_p]),
+    "ic_observables": (C.c_int, [C.c_void_p, C.POINTER(ic_obs)]),
+    "ic_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "ic_debug_recompute": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
+    "ic_thresholds": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(C.c_uint32)]),
+    "ic_schedule": (C.c_int, [C.c_void_p, C.c_uint64, C.POINTER(C.c_int32)]),
+    "ic_sweep_count": (C.c_int64, [C.c_void_p]),
+    "ic_charge": (C.c_int64, [C.c_void_p]),
+    "ic_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
+    "ic_launch_count": (C.c_int64, [C.c_void_p]),
+    "ic_destroy": (C.c_int, [C.c_void_p]),
+    "ic_strerror": (C.c_char_p, [C.c_int]),
+}
+
+
+def _load():
+    path = _build.build()          # raises if nvcc fails; never falls back to anything else
+    lib = C.CDLL(path)
+    for name, (res, args) in EXPORTS.items():
+        fn = getattr(lib, name)    # AttributeError if the library does not export it
+        fn.restype, fn.argtypes = res, args
+    return lib, path
+
+
+lib, LIB_PATH = _load()
+
+
+class IcError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__(f"{where}: {lib.ic_strerror(code).decode()} (code {code})")
+
+
+def _check(code, where):
+    if code != IC_OK:
+        raise IcError(code, where)
+
+
+class Sim:
+    """`replicas` copies of an L x L lattice on the current CUDA device; thin wrapper over the ic_* calls."""
+
+    def __init__(self, L, n, delta, V, J, seed, replicas=1, bits_per_site=8, device=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2301_11735_b200 needs a CUDA device (there is no CPU path)")
+        self.torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self.L, self.N, self.replicas, self.bits = int(L), int(L) * int(L), int(replicas), int(bits_per_site)
+        nbytes = lib.ic_workspace_bytes(self.L, self.replicas, self.bits)
+        if nbytes == 0:
+            raise IcError(IC_ERR_SIZE, "ic_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            aligned = (base + 255) & ~255
+            self.stream = torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            _check(lib.ic_create(C.byref(h), self.L, float(n), float(delta), float(V), float(J), int(seed), self.replicas,
+                                 self.bits, C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream)), "ic_create")
+        self.h = h
+        self.workspace_bytes = nbytes
+
+    # -- the boundary, one method per entry point -------------------------------------------------------------
+    def init_charges(self, replica, nplus, nminus):
+        _check(lib.ic_init_charges(self.h, int(replica), int(nplus), int(nminus)), "ic_init_charges")
+
+    def set_state(self, replica, codes):
+        """codes: numpy int8 [L, L] (or a pinned torch CPU tensor) of public site codes."""
+        if hasattr(codes, "data_ptr"):
+            assert codes.device.type == "cpu" and codes.is_contiguous() and codes.numel() == self.N and codes.element_size() == 1
+            ptr = codes.data_ptr()
+        else:
+            codes = np.ascontiguousarray(codes, dtype=np.int8)
+            assert codes.size == self.N
+            ptr = codes.ctypes.data
+        _check(lib.ic_set_state(self.h, int(replica), C.c_void_p(ptr)), "ic_set_state")
+
+    def _T(self, T):
+        arr = np.ascontiguousarray(np.broadcast_to(np.asarray(T, dtype=np.float64), (self.replicas,)))
+        return arr, arr.ctypes.data_as(C.POINTER(C.c_double))
+
+    def sweep(self, T, nsweeps):
+        arr, p = self._T(T)
+        _check(lib.ic_sweep(self.h, p, int(nsweeps)), "ic_sweep")
+
+    def sweep_trace(self, T, nsweeps):
+        """Returns a device int64 tensor [nsweeps, replicas, 6] = (n2, bV, bJ, M, Ms, Q) after every sweep."""
+        arr, p = self._T(T)
+        tr = self.torch.empty((int(nsweeps), self.replicas, 6), dtype=self.torch.int64, device=self.device)
+        _check(lib.ic_sweep_trace(self.h, p, int(nsweeps), C.c_void_p(tr.data_ptr())), "ic_sweep_trace")
+        return tr
+
+    def reset_observables(self):
+        _check(lib.ic_reset_observables(self.h), "ic_reset_observables")
+
+    def observables(self):
+        out = (ic_obs * self.replicas)()
+        _check(lib.ic_observables(self.h, out), "ic_observables")
+        return [{f: getattr(o, f) for f, _ in ic_obs._fields_} for o in out]
+
+    def state(self, replica=0, out=None):
+        if out is None:
+            out = np.empty((self.L, self.L), dtype=np.int8)
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        _check(lib.ic_state(self.h, int(replica), C.c_void_p(ptr)), "ic_state")
+        return out
+
+    def debug_recompute(self, replica=0):
+        out = (C.c_int64 * 6)()
+        _check(lib.ic_debug_recompute(self.h, int(replica), out), "ic_debug_recompute")
+        return np.array(list(out), dtype=np.int64)
+
+    def thresholds(self, T):
+        out = np.zeros(IC_N_CLASSES, dtype=np.uint32)
+        _check(lib.ic_thresholds(self.h, float(T), out.ctypes.data_as(C.POINTER(C.c_uint32))), "ic_thresholds")
+        return out
+
+    def schedule(self, sweep):
+        out = (C.c_int32 * 4)()
+        _check(lib.ic_schedule(self.h, int(sweep), out), "ic_schedule")
+        return tuple(out)
+
+    def set_variant(self, variant):
+        _check(lib.ic_set_variant(self.h, int(variant)), "ic_set_variant")
+
+    @property
+    def sweep_count(self):
+        return int(lib.ic_sweep_count(self.h))
+
+    @property
+    def Q(self):
+        return int(lib.ic_charge(self.h))
+
+    @property
+    def launch_count(self):
+        return int(lib.ic_launch_count(self.h))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib.ic_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,426 @@
+// ic_api.cu -- host side of libic_b200: the C ABI of include/ic.h.
+//
+// Validates arguments, carves the caller's workspace, builds the acceptance-threshold tables (U2) and the
+// O(1) schedule parameters of each sweep (U4), and launches the sm_100a kernels.  No lattice arithmetic runs
+// on the host except stage 1 of the algorithm (the initial configuration with the prescribed
+// charge), which is a sequential selection and belongs to ic_create, not to the sweep.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <thread>
+#include <vector>
+
+#include "../../include/ic.h"
+#include "ic_common.cuh"
+#include "ic_kernels_ref.cuh"
+
+using namespace ic;
+
+struct ic_ctx {
+  int L, logL, replicas, bits, variant;
+  long long N, Q;
+  double n, delta, V, J;
+  uint64_t seed, sweep;
+  cudaStream_t stream;
+  // device (inside the caller's workspace)
+  char* lattice; long long lat_stride;
+  uint32_t* d_thr; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
+  // host (pinned)
+  uint32_t* h_thr; ReplicaObs* h_obs;
+  cudaEvent_t thr_copied;
+  std::vector<double>* lastT; bool have_T;
+  long long launches;
+};
+
+static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "%s: %s", what, cudaGetErrorString(e));
+  return IC_ERR_CUDA;
+}
+#define IC_CUDA(call)                                        \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);      \
+  } while (0)
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+static bool valid_dims(int L, int replicas, int bits) {
+  return L >= 4 && L <= 65536 && (L & (L - 1)) == 0 && replicas >= 1 && replicas <= 65535 && (bits == 8 || bits == 2);
+}
+static size_t lattice_bytes(int L, int bits) { return (size_t)L * L * bits / 8; }
+
+extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
+  if (!valid_dims(L, replicas, bits)) return 0;
+  size_t b = 0;
+  b += align256(lattice_bytes(L, bits)) * (size_t)replicas;       // lattices
+  b += align256((size_t)replicas * THR_STRIDE * sizeof(uint32_t)); // thresholds
+  b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
+  b += 256;                                                        // scratch for ic_debug_recompute
+  b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
+  return b;
+}
+
+// U2: acceptance threshold of a class at temperature T.  Metropolis min(1, exp(-dE/T)) as a 29-bit
+// integer; IEEE fp64, the C library's exp, no FMA contraction (built with -ffp-contract=off).
+static uint32_t threshold29(double delta, double V, double quarterJ, int dn2, int dV, int dJ, double T) {
+  const double dE = (delta * (double)dn2 + V * (double)dV) + quarterJ * (double)dJ;
+  if (dE <= 0.0) return 1u << 29;
+  double t = std::floor(std::exp(-dE / T) * 536870912.0);
+  if (t < 1.0) t = 1.0;
+  if (t > 536870911.0) t = 536870911.0;
+  return (uint32_t)t;
+}
+static void build_thresholds(const ic_ctx* c, double T, uint32_t* out) {
+  const double qJ = 0.25 * c->J;
+  for (int a = -1; a <= 1; ++a)
+    for (int v = -16; v <= 16; ++v)
+      for (int j = -16; j <= 16; ++j) out[class_index(2 * a, v, j)] = threshold29(c->delta, c->V, qJ, 2 * a, v, j, T);
+}
+
+// U4: parameters of sweep s, from Philox(ctr = (0, 0, s, TAG_SCHED), key = seed); the same for all replicas.
+static void schedule_params(int L, uint64_t seed, uint64_t sweep, int32_t out4[4]) {
+  u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, (uint32_t)seed, (uint32_t)(seed >> 32));
+  if ((sweep & 1) == 0) {   // FAR sweep: odd XOR masks, partner(x,y) = (x^mx, y^my)
+    out4[0] = 0; out4[1] = (int32_t)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); out4[2] = (int32_t)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1);
+  } else {                  // NEAR sweep: dominoes, orientation and offset
+    out4[0] = 1; out4[1] = (int32_t)(z.v[0] & 1u); out4[2] = (int32_t)(z.v[1] & 3u);
+  }
+  out4[3] = 0;
+}
+
+// U0, stage 1: all sites magnetic with random sigma, then nplus sites S=+1 and nminus sites S=-1
+// at distinct random sites by selection sampling over the counter-based stream (seed, replica, TAG_INIT).
+static void stage1_init(int8_t* code, long long N, long long nplus, long long nminus, uint64_t seed, int replica) {
+  const long long CH = 1LL << 20;
+  unsigned hw = std::thread::hardware_concurrency();
+  const int nth = (int)std::max(1u, std::min(hw ? hw : 1u, 32u));
+  std::vector<uint32_t> w(3 * (size_t)std::min(CH, N));
+  const long long K = nplus + nminus;
+  long long picked = 0, plus = 0;
+  for (long long base = 0; base < N; base += CH) {
+    const long long cnt = std::min(CH, N - base);
+    auto fill = [&](long long lo, long long hi) {
+      for (long long k = lo; k < hi; ++k) {
+        const long long i = base + k;
+        u32x4 z = philox4x32_10((uint32_t)(i & 0xFFFFFFFFLL), (uint32_t)(i >> 32), 0u,
+                                ((uint32_t)replica & 0x0FFFFFFFu) | (TAG_INIT << 28), (uint32_t)seed, (uint32_t)(seed >> 32));
+        w[3 * k] = z.v[0]; w[3 * k + 1] = z.v[1]; w[3 * k + 2] = z.v[2];
+      }
+    };
+    if (cnt < 65536 || nth == 1) fill(0, cnt);
+    else {
+      std::vector<std::thread> th;
+      for (int t = 0; t < nth; ++t) th.emplace_back(fill, cnt * t / nth, cnt * (t + 1) / nth);
+      for (auto& t : th) t.join();
+    }
+    for (long long k = 0; k < cnt; ++k) {
+      const long long i = base + k;
+      int c = (w[3 * k] & 1u) ? 1 : 0;
+      if ((long long)(((uint64_t)w[3 * k + 1] * (uint64_t)(N - i)) >> 32) < K - picked) {
+        if ((long long)(((uint64_t)w[3 * k + 2] * (uint64_t)(K - picked)) >> 32) < nplus - plus) { c = 2; ++plus; }
+        else c = 3;
+        ++picked;
+      }
+      code[i] = (int8_t)c;
+    }
+  }
+}
+
+__global__ void k_store_ints(ReplicaObs* o, const long long* s8) {
+  o->n2 = s8[0]; o->bV = s8[1]; o->bJ = s8[2]; o->M = s8[3]; o->Ms = s8[4]; o->Q = s8[5];
+}
+
+static int recompute_into_scratch(ic_ctx* c, int replica) {
+  IC_CUDA(cudaMemsetAsync(c->d_scratch8, 0, 64, c->stream));
+  const void* lat = c->lattice + (long long)replica * c->lat_stride;
+  const int blocks = (int)std::min<long long>((c->N + 255) / 256, 148 * 8);
+  if (c->bits == 8) k_recompute<8><<<blocks, 256, 0, c->stream>>>(lat, c->L, c->logL, c->d_scratch8);
+  else k_recompute<2><<<blocks, 256, 0, c->stream>>>(lat, c->L, c->logL, c->d_scratch8);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
+// Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.
+static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
+  char* lat = c->lattice + (long long)replica * c->lat_stride;
+  if (c->bits == 8) {
+    IC_CUDA(cudaMemcpyAsync(lat, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
+  } else {
+    IC_CUDA(cudaMemcpyAsync(c->d_stage, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
+    const long long n16 = c->N / 16;
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 8);
+    k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+  }
+  int rc = recompute_into_scratch(c, replica);
+  if (rc != IC_OK) return rc;
+  k_store_ints<<<1, 1, 0, c->stream>>>(&c->d_obs[replica], c->d_scratch8);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
+extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, double J, uint64_t seed, int replicas,
+                         int bits, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return IC_ERR_NULL;
+  *out = nullptr;
+  if (!valid_dims(L, replicas, bits)) return IC_ERR_SIZE;
+  if (!std::isfinite(n) || !std::isfinite(delta) || !std::isfinite(V) || !std::isfinite(J) || std::fabs(n) > 1.0) return IC_ERR_PARAM;
+  const size_t need = ic_workspace_bytes(L, replicas, bits);
+  if (!d_workspace || workspace_bytes < need || ((uintptr_t)d_workspace & 255) != 0) return IC_ERR_WORKSPACE;
+
+  ic_ctx* c = new (std::nothrow) ic_ctx();
+  if (!c) return IC_ERR_NULL;
+  c->L = L; c->logL = 0; while ((1 << c->logL) < L) c->logL++;
+  c->replicas = replicas; c->bits = bits; c->variant = 0;
+  c->N = (long long)L * L; c->Q = std::llround(n * (double)c->N);
+  c->n = n; c->delta = delta; c->V = V; c->J = J; c->seed = seed; c->sweep = 0;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->launches = 0; c->have_T = false; c->lastT = new std::vector<double>((size_t)replicas, 0.0);
+  char* p = (char*)d_workspace;
+  c->lattice = p; c->lat_stride = (long long)align256(lattice_bytes(L, bits)); p += (size_t)c->lat_stride * replicas;
+  c->d_thr = (uint32_t*)p; p += align256((size_t)replicas * THR_STRIDE * sizeof(uint32_t));
+  c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
+  c->d_scratch8 = (long long*)p; p += 256;
+  c->d_stage = (int8_t*)p;
+  c->h_thr = nullptr; c->h_obs = nullptr; c->thr_copied = nullptr;
+
+  auto fail = [&](int rc) { ic_destroy(c); return rc; };
+  if (cudaMallocHost((void**)&c->h_thr, (size_t)replicas * THR_STRIDE * sizeof(uint32_t)) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost(thresholds)"));
+  if (cudaMallocHost((void**)&c->h_obs, (size_t)replicas * sizeof(ReplicaObs)) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost(observables)"));
+  if (cudaEventCreateWithFlags(&c->thr_copied, cudaEventDisableTiming) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaEventCreate"));
+  memset(c->h_thr, 0, (size_t)replicas * THR_STRIDE * sizeof(uint32_t));
+  cudaError_t e = cudaMemsetAsync(c->d_obs, 0, (size_t)replicas * sizeof(ReplicaObs), c->stream);
+  if (e != cudaSuccess) return fail(cuda_fail(e, "cudaMemsetAsync(observables)"));
+
+  // stage 1 for every replica
+  std::vector<int8_t> codes((size_t)c->N);
+  const long long nplus = c->Q > 0 ? c->Q : 0, nminus = c->Q < 0 ? -c->Q : 0;
+  for (int r = 0; r < replicas; ++r) {
+    stage1_init(codes.data(), c->N, nplus, nminus, seed, r);
+    int rc = upload_state(c, r, codes.data());
+    if (rc != IC_OK) return fail(rc);
+    e = cudaStreamSynchronize(c->stream);   // codes is reused for the next replica
+    if (e != cudaSuccess) return fail(cuda_fail(e, "cudaStreamSynchronize(init)"));
+  }
+  *out = c;
+  return IC_OK;
+}
+
+extern "C" int ic_destroy(ic_ctx* c) {
+  if (!c) return IC_ERR_NULL;
+  if (c->stream || true) cudaStreamSynchronize(c->stream);
+  if (c->h_thr) cudaFreeHost(c->h_thr);
+  if (c->h_obs) cudaFreeHost(c->h_obs);
+  if (c->thr_copied) cudaEventDestroy(c->thr_copied);
+  delete c->lastT;
+  delete c;
+  return IC_OK;
+}
+
+extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nminus) {
+  if (!c) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  if (nplus < 0 || nminus < 0 || nplus + nminus > c->N || nplus - nminus != c->Q) return IC_ERR_CHARGE;
+  std::vector<int8_t> codes((size_t)c->N);
+  stage1_init(codes.data(), c->N, nplus, nminus, c->seed, replica);
+  int rc = upload_state(c, replica, codes.data());
+  if (rc != IC_OK) return rc;
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  return IC_OK;
+}
+
+extern "C" int ic_set_state(ic_ctx* c, int replica, const int8_t* h_codes) {
+  if (!c || !h_codes) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  // every code in 0..3 and sum S == Q, eight sites at a time: bit1 = charge, bit0 = sign
+  long long nch = 0, nneg = 0; uint64_t bad = 0;
+  const long long N = c->N;   // N >= 16 and a multiple of 8
+  for (long long i = 0; i < N; i += 8) {
+    uint64_t v; memcpy(&v, h_codes + i, 8);
+    bad |= v & 0xFCFCFCFCFCFCFCFCull;
+    const uint64_t ch = (v >> 1) & 0x0101010101010101ull;
+    nch += __builtin_popcountll(ch);
+    nneg += __builtin_popcountll(ch & v);
+  }
+  if (bad) return IC_ERR_CHARGE;
+  if ((nch - nneg) - nneg != c->Q) return IC_ERR_CHARGE;
+  int rc = upload_state(c, replica, h_codes);
+  if (rc != IC_OK) return rc;
+  IC_CUDA(cudaStreamSynchronize(c->stream));   // h_codes may be pageable and is the caller's to reuse
+  return IC_OK;
+}
+
+extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
+  if (!c || !h_out) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  const char* lat = c->lattice + (long long)replica * c->lat_stride;
+  if (c->bits == 8) {
+    IC_CUDA(cudaMemcpyAsync(h_out, lat, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
+  } else {
+    const long long n16 = c->N / 16;
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 8);
+    k_unpack2<<<blocks, 256, 0, c->stream>>>((const uint32_t*)lat, c->d_stage, n16);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+    IC_CUDA(cudaMemcpyAsync(h_out, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
+  }
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  return IC_OK;
+}
+
+static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
+  const long long npairs = c->N / 4;
+  dim3 grid((unsigned)((npairs + 255) / 256), (unsigned)c->replicas);
+  if (c->bits == 8) k_ref_phase<8><<<grid, 256, 0, c->stream>>>(a);
+  else k_ref_phase<2><<<grid, 256, 0, c->stream>>>(a);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
+static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_trace) {
+  if (!c || !h_T) return IC_ERR_NULL;
+  if (nsweeps < 0 || c->sweep + (uint64_t)nsweeps >= (1ull << 31)) return IC_ERR_PARAM;
+  for (int r = 0; r < c->replicas; ++r)
+    if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
+  if (nsweeps == 0) return IC_OK;
+
+  // thresholds: rebuilt and uploaded only when a temperature changed
+  bool changed = !c->have_T;
+  for (int r = 0; r < c->replicas && !changed; ++r) changed = (*c->lastT)[r] != h_T[r];
+  if (changed) {
+    IC_CUDA(cudaEventSynchronize(c->thr_copied));   // the previous upload has left the pinned buffer
+    for (int r = 0; r < c->replicas; ++r) {
+      if (c->have_T && (*c->lastT)[r] == h_T[r]) continue;
+      build_thresholds(c, h_T[r], c->h_thr + (size_t)r * THR_STRIDE);
+      (*c->lastT)[r] = h_T[r];
+    }
+    IC_CUDA(cudaMemcpyAsync(c->d_thr, c->h_thr, (size_t)c->replicas * THR_STRIDE * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
+    IC_CUDA(cudaEventRecord(c->thr_copied, c->stream));
+    c->have_T = true;
+  }
+
+  PhaseArgs a;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
+  a.L = c->L; a.logL = c->logL; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
+  const double qJ = 0.25 * c->J;
+  for (int64_t s = 0; s < nsweeps; ++s) {
+    int32_t par[4];
+    schedule_params(c->L, c->seed, c->sweep, par);
+    a.type = par[0]; a.p1 = par[1]; a.p2 = par[2];
+    for (int phase = 0; phase < 2; ++phase) {
+      a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
+      int rc = launch_phase_ref(c, a);
+      if (rc != IC_OK) return rc;
+    }
+    k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ,
+                                                               d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+    c->sweep += 1;
+  }
+  return IC_OK;
+}
+
+extern "C" int ic_sweep(ic_ctx* c, const double* h_T, int64_t nsweeps) { return sweep_impl(c, h_T, nsweeps, nullptr); }
+extern "C" int ic_sweep_trace(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_trace) {
+  if (!d_trace && nsweeps > 0) return IC_ERR_NULL;
+  return sweep_impl(c, h_T, nsweeps, d_trace);
+}
+
+__global__ void k_reset_sums(ReplicaObs* obs, int replicas) {
+  int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= replicas) return;
+  ReplicaObs* o = &obs[r];
+  o->nmeas = 0; o->sumE = o->sumE2 = o->sumM = o->sumM2 = o->sumAbsM = o->sumMs = o->sumMs2 = o->sumAbsMs = 0.0;
+}
+
+extern "C" int ic_reset_observables(ic_ctx* c) {
+  if (!c) return IC_ERR_NULL;
+  k_reset_sums<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
+extern "C" int ic_observables(ic_ctx* c, ic_obs* h_out) {
+  if (!c || !h_out) return IC_ERR_NULL;
+  IC_CUDA(cudaMemcpyAsync(c->h_obs, c->d_obs, (size_t)c->replicas * sizeof(ReplicaObs), cudaMemcpyDeviceToHost, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  for (int r = 0; r < c->replicas; ++r) {
+    const ReplicaObs& o = c->h_obs[r];
+    ic_obs& q = h_out[r];
+    q.nmeas = o.nmeas; q.n2 = o.n2; q.bV = o.bV; q.bJ = o.bJ; q.M = o.M; q.Ms = o.Ms; q.Q = o.Q;
+    q.sumE = o.sumE; q.sumE2 = o.sumE2; q.sumM = o.sumM; q.sumM2 = o.sumM2; q.sumAbsM = o.sumAbsM;
+    q.sumMs = o.sumMs; q.sumMs2 = o.sumMs2; q.sumAbsMs = o.sumAbsMs;
+    const double T = c->have_T ? (*c->lastT)[r] : 0.0;
+    q.T = T; q.C = q.chi_u = q.chi_s = 0.0;
+    if (T > 0.0) {   // C = (<E^2> - <E>^2)/(N k T^2), k = 1; chi: DESIGN.md G9
+      const double cnt = (double)(o.nmeas > 0 ? o.nmeas : 1), Nd = (double)c->N;
+      const double mE = o.sumE / cnt, mE2 = o.sumE2 / cnt, mM = o.sumM / cnt, mM2 = o.sumM2 / cnt;
+      const double mMs = o.sumMs / cnt, mMs2 = o.sumMs2 / cnt;
+      q.C = (mE2 - mE * mE) / (Nd * T * T);
+      q.chi_u = (mM2 - mM * mM) / (Nd * T);
+      q.chi_s = (mMs2 - mMs * mMs) / (Nd * T);
+    }
+  }
+  return IC_OK;
+}
+
+extern "C" int ic_debug_recompute(ic_ctx* c, int replica, int64_t* out6) {
+  if (!c || !out6) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  int rc = recompute_into_scratch(c, replica);
+  if (rc != IC_OK) return rc;
+  long long h[8];
+  IC_CUDA(cudaMemcpyAsync(h, c->d_scratch8, 64, cudaMemcpyDeviceToHost, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 6; ++k) out6[k] = h[k];
+  return IC_OK;
+}
+
+extern "C" int ic_thresholds(ic_ctx* c, double T, uint32_t* h_out) {
+  if (!c || !h_out) return IC_ERR_NULL;
+  if (!(T > 0.0) || !std::isfinite(T)) return IC_ERR_PARAM;
+  std::vector<uint32_t> tmp(THR_STRIDE);
+  build_thresholds(c, T, tmp.data());
+  memcpy(h_out, tmp.data(), sizeof(uint32_t) * N_CLASSES);
+  return IC_OK;
+}
+
+extern "C" int ic_schedule(ic_ctx* c, uint64_t sweep, int32_t* out4) {
+  if (!c || !out4) return IC_ERR_NULL;
+  if (sweep >= (1ull << 31)) return IC_ERR_PARAM;
+  schedule_params(c->L, c->seed, sweep, out4);
+  return IC_OK;
+}
+
+extern "C" int64_t ic_sweep_count(const ic_ctx* c) { return c ? (int64_t)c->sweep : -1; }
+extern "C" int64_t ic_charge(const ic_ctx* c) { return c ? (int64_t)c->Q : 0; }
+extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->launches : -1; }
+
+extern "C" int ic_set_variant(ic_ctx* c, int variant) {
+  if (!c) return IC_ERR_NULL;
+  if (variant < 0 || variant > 1) return IC_ERR_PARAM;
+  c->variant = variant;
+  return IC_OK;
+}
+
+extern "C" const char* ic_strerror(int code) {
+  switch (code) {
+    case IC_OK: return "ok";
+    case IC_ERR_NULL: return "a required pointer is NULL";
+    case IC_ERR_SIZE: return "invalid size: L must be a power of two in [4, 65536], replicas >= 1, bits_per_site 8 or 2, replica in range";
+    case IC_ERR_PARAM: return "invalid parameter: |n| <= 1, finite Delta, V, J, T > 0, nsweeps >= 0, sweep counter < 2^31";
+    case IC_ERR_WORKSPACE: return "workspace is NULL, too small (see ic_workspace_bytes) or not 256-byte aligned";
+    case IC_ERR_CHARGE: return "state rejected: a code outside 0..3 or sum S != Q";
+    case IC_ERR_CUDA: return g_cuda_msg;
+    default: return "unknown error code";
+  }
+}

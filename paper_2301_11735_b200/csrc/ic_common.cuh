@@ -1,0 +1,78 @@
+// ic_common.cuh -- definitions shared by the host control code and the sm_100a kernels of libic_b200.
+//
+// Notation follows the paper (arXiv:2301.11735): site state S = +-1 (charge) or s = +-1/2 with S = 0
+// (magnetic), sigma = 2(1-S^2)s.  Public site code c: 0 sigma=+1, 1 sigma=-1, 2 S=+1, 3 S=-1.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#define IC_HD __host__ __device__ __forceinline__
+
+namespace ic {
+
+// ---------------------------------------------------------------------------------------------------
+// Random numbers: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), counter-based, keyed by the seed.
+// The paper only says pairs and configurations are "randomly selected"; U3.
+// Counter = (c0, c1, c2, replica | tag << 28).
+// ---------------------------------------------------------------------------------------------------
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
+enum : uint32_t { TAG_UPDATE = 0, TAG_SCHED = 1, TAG_INIT = 2 };
+
+struct u32x4 { uint32_t v[4]; };
+
+IC_HD void mulhilo(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
+#ifdef __CUDA_ARCH__
+  lo = a * b; hi = __umulhi(a, b);
+#else
+  uint64_t p = (uint64_t)a * (uint64_t)b; lo = (uint32_t)p; hi = (uint32_t)(p >> 32);
+#endif
+}
+
+IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int round = 0; round < 10; ++round) {
+    uint32_t h0, l0, h1, l1;
+    mulhilo(PHILOX_M0, c0, h0, l0);
+    mulhilo(PHILOX_M1, c2, h1, l1);
+    c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+    k0 += PHILOX_W0; k1 += PHILOX_W1;
+  }
+  u32x4 r; r.v[0] = c0; r.v[1] = c1; r.v[2] = c2; r.v[3] = c3; return r;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Site code -> S, sigma.  bit1 = "is a charge", bit0 = "negative".
+// ---------------------------------------------------------------------------------------------------
+IC_HD int S_of(int c) { return (c & 2) ? 1 - 2 * (c & 1) : 0; }
+IC_HD int sg_of(int c) { return (c & 2) ? 0 : 1 - 2 * (c & 1); }
+
+// Acceptance class of a move (E_Delta, E_V, E_J): dn2 in {-2,0,2}, dV, dJ in [-16,16].
+constexpr int N_CLASSES = 3 * 33 * 33;   // 3267
+constexpr int THR_STRIDE = 3328;         // table stride per replica (multiple of 64 words)
+IC_HD int class_index(int dn2, int dV, int dJ) { return ((dn2 / 2 + 1) * 33 + (dV + 16)) * 33 + (dJ + 16); }
+
+// Per-replica record in device memory: exact integers, then the fp64 sums of U5.
+struct ReplicaObs {
+  long long n2, bV, bJ, M, Ms, Q;      // current exact integers (updated by the phase kernels)
+  long long nmeas, pad0;
+  double sumE, sumE2, sumM, sumM2, sumAbsM, sumMs, sumMs2, sumAbsMs;
+};
+static_assert(sizeof(ReplicaObs) == 128, "ReplicaObs layout");
+
+// Parameters of one phase of one sweep (schedule S1, U4), the same for all replicas
+// (precedent: identical maps for all lattice copies).
+struct PhaseArgs {
+  void* lattice;                 // [replicas][lat_stride bytes]
+  const uint32_t* thr;           // [replicas][THR_STRIDE] thresholds t29
+  ReplicaObs* obs;               // [replicas]
+  long long lat_stride;          // bytes per replica
+  int L, logL;
+  int type;                      // 0 FAR (partner = (x^mx, y^my)), 1 NEAR (dominoes)
+  int p1, p2;                    // FAR: mx, my.  NEAR: orientation (0 horizontal, 1 vertical), offset 0..3
+  int phase;                     // 0 or 1
+  uint32_t c2;                   // 2*sweep + phase
+  uint32_t key0, key1;           // Philox key = seed
+};
+
+}  // namespace ic

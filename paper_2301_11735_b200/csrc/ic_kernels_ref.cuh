@@ -1,0 +1,210 @@
+// ic_kernels_ref.cuh -- variant 1: one thread per coupled pair, lattice in global memory.
+//
+// The plain CUDA statement of the pair update (sec. 3.1) under schedule S1 (U4).
+// It runs any power-of-two L >= 4 at 8 or 2 bits per site and is the in-library cross-check for the tiled
+// and resident kernels; it is also what tiny lattices (L < 16) use.  Each thread recomputes the Philox block
+// of its group of four pairs and keeps one word.
+#pragma once
+#include "ic_common.cuh"
+
+namespace ic {
+
+template <int BITS>
+struct Sites {
+  // BITS == 8: one byte per site.  BITS == 2: 16 sites per 32-bit word, site i at bits 2(i&15) of word i>>4.
+  static __device__ __forceinline__ int load(const void* base, long long i) {
+    if (BITS == 8) return ((const int8_t*)base)[i];
+    return (((const uint32_t*)base)[i >> 4] >> (2 * (int)(i & 15))) & 3;
+  }
+  // Sites written in one phase are distinct, but with BITS == 2 several threads share a word: xor the change in.
+  static __device__ __forceinline__ void store(void* base, long long i, int oldc, int newc) {
+    if (BITS == 8) ((int8_t*)base)[i] = (int8_t)newc;
+    else atomicXor(&((uint32_t*)base)[i >> 4], (uint32_t)(oldc ^ newc) << (2 * (int)(i & 15)));
+  }
+};
+
+// Sum of five per-thread integers over the block, then one atomicAdd per value into the replica record.
+__device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV, int dJ, int dM, int dMs) {
+  __shared__ int red[5][32];
+  const unsigned full = 0xFFFFFFFFu;
+  dn2 = __reduce_add_sync(full, dn2); dV = __reduce_add_sync(full, dV); dJ = __reduce_add_sync(full, dJ);
+  dM = __reduce_add_sync(full, dM); dMs = __reduce_add_sync(full, dMs);
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+  if (lane == 0) { red[0][warp] = dn2; red[1][warp] = dV; red[2][warp] = dJ; red[3][warp] = dM; red[4][warp] = dMs; }
+  __syncthreads();
+  if (warp == 0) {
+    int v[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) v[k] = __reduce_add_sync(full, lane < nwarp ? red[k][lane] : 0);
+    if (lane == 0) {
+      if (v[0]) atomicAdd((unsigned long long*)&o->n2, (unsigned long long)(long long)v[0]);
+      if (v[1]) atomicAdd((unsigned long long*)&o->bV, (unsigned long long)(long long)v[1]);
+      if (v[2]) atomicAdd((unsigned long long*)&o->bJ, (unsigned long long)(long long)v[2]);
+      if (v[3]) atomicAdd((unsigned long long*)&o->M, (unsigned long long)(long long)v[3]);
+      if (v[4]) atomicAdd((unsigned long long*)&o->Ms, (unsigned long long)(long long)v[4]);
+    }
+  }
+}
+
+template <int BITS>
+__global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
+  const int L = A.L, logL = A.logL, mask = L - 1;
+  const int r = blockIdx.y;
+  const long long npairs = ((long long)L * L) >> 2;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  void* lat = (char*)A.lattice + (long long)r * A.lat_stride;
+  int dn2 = 0, dV = 0, dJ = 0, dM = 0, dMs = 0;
+  if (t < npairs) {
+    // --- which pair (schedule S1) and which random word ---------------------------------------------
+    int xa, ya, xb, yb, adj; uint32_t c0, word;
+    if (A.type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
+      int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
+      xa = 2 * i; ya = 2 * j + A.phase; xb = xa ^ A.p1; yb = ya ^ A.p2; adj = 0;
+      c0 = (uint32_t)xa >> 3; word = ((uint32_t)xa >> 1) & 3u;
+    } else if (A.p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
+      int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
+      xa = ((A.p2 + 2 * ((ya + A.phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
+      uint32_t rank = (uint32_t)xb >> 2; c0 = rank >> 2; word = rank & 3u;
+    } else {                           // NEAR, vertical dominoes
+      xa = (int)(t & mask); int jy = (int)(t >> logL);
+      ya = ((A.p2 + 2 * ((xa + A.phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
+      uint32_t rank = (uint32_t)xa >> 1; c0 = rank >> 2; word = rank & 3u;
+    }
+    u32x4 rnd = philox4x32_10(c0, (uint32_t)ya, A.c2, (uint32_t)r | (TAG_UPDATE << 28), A.key0, A.key1);
+    uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
+
+    // --- proposal: same pair charge q, configuration r of the paper's list ----------
+    const long long ia = ((long long)ya << logL) + xa, ib = ((long long)yb << logL) + xb;
+    const int ca = Sites<BITS>::load(lat, ia), cb = Sites<BITS>::load(lat, ib);
+    const int q = S_of(ca) + S_of(cb);
+    const int rr = (int)(w & 7u);
+    int na = ca, nb = cb;
+    if (q == 0) {
+      // (S+,S-) (S-,S+) (s+,s+) (s-,s-) (s+,s-) (s-,s+); rr = 6,7: nothing proposed
+      switch (rr) {
+        case 0: na = 2; nb = 3; break;
+        case 1: na = 3; nb = 2; break;
+        case 2: na = 0; nb = 0; break;
+        case 3: na = 1; nb = 1; break;
+        case 4: na = 0; nb = 1; break;
+        case 5: na = 1; nb = 0; break;
+        default: na = ca; nb = cb; break;
+      }
+    } else if (q == 1 || q == -1) {
+      const int C = q > 0 ? 2 : 3;     // (C,s+) (C,s-) (s+,C) (s-,C)
+      switch (rr & 3) {
+        case 0: na = C; nb = 0; break;
+        case 1: na = C; nb = 1; break;
+        case 2: na = 0; nb = C; break;
+        default: na = 1; nb = C; break;
+      }
+    }
+    if (na != ca || nb != cb) {
+      // --- neighbour sums over the four slots of a and of b, current lattice ----------
+      const int xl = (xa - 1) & mask, xr = (xa + 1) & mask, yu = (ya - 1) & mask, yd = (ya + 1) & mask;
+      const int c1 = Sites<BITS>::load(lat, ((long long)ya << logL) + xl), c2 = Sites<BITS>::load(lat, ((long long)ya << logL) + xr);
+      const int c3 = Sites<BITS>::load(lat, ((long long)yu << logL) + xa), c4 = Sites<BITS>::load(lat, ((long long)yd << logL) + xa);
+      const int xl2 = (xb - 1) & mask, xr2 = (xb + 1) & mask, yu2 = (yb - 1) & mask, yd2 = (yb + 1) & mask;
+      const int e1 = Sites<BITS>::load(lat, ((long long)yb << logL) + xl2), e2 = Sites<BITS>::load(lat, ((long long)yb << logL) + xr2);
+      const int e3 = Sites<BITS>::load(lat, ((long long)yu2 << logL) + xb), e4 = Sites<BITS>::load(lat, ((long long)yd2 << logL) + xb);
+      const int nSa = S_of(c1) + S_of(c2) + S_of(c3) + S_of(c4), nGa = sg_of(c1) + sg_of(c2) + sg_of(c3) + sg_of(c4);
+      const int nSb = S_of(e1) + S_of(e2) + S_of(e3) + S_of(e4), nGb = sg_of(e1) + sg_of(e2) + sg_of(e3) + sg_of(e4);
+      // --- dE class: eq. (4) distant / eq. (5) neighbouring sites, spin term as in DESIGN.md G1 ------
+      const int dSa = S_of(na) - S_of(ca), dSb = S_of(nb) - S_of(cb);
+      const int dGa = sg_of(na) - sg_of(ca), dGb = sg_of(nb) - sg_of(cb);
+      const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
+      const int e_v = dSa * nSa + dSb * nSb + adj * dSa * dSb;
+      const int e_j = dGa * nGa + dGb * nGb + adj * dGa * dGb;
+      const uint32_t t29 = __ldg(&A.thr[(long long)r * THR_STRIDE + class_index(e_d, e_v, e_j)]);
+      if ((w >> 3) < t29) {            // Metropolis min(1, exp(-dE/T)) as an integer compare
+        Sites<BITS>::store(lat, ia, ca, na);
+        Sites<BITS>::store(lat, ib, cb, nb);
+        dn2 = e_d; dV = e_v; dJ = e_j; dM = dGa + dGb;
+        dMs = (((xa + ya) & 1) ? -dGa : dGa) + (((xb + yb) & 1) ? -dGb : dGb);
+      }
+    }
+  }
+  block_accumulate(&A.obs[r], dn2, dV, dJ, dM, dMs);
+}
+
+// U5: after a sweep, E = Delta*n2 + V*bV + (J/4)*bJ and the running sums, one thread per
+// replica, IEEE fp64 with one rounding per operation (no FMA contraction: explicit _rn intrinsics).
+__global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row) {
+  int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= replicas) return;
+  ReplicaObs* o = &obs[r];
+  const double E = __dadd_rn(__dadd_rn(__dmul_rn(delta, (double)o->n2), __dmul_rn(V, (double)o->bV)),
+                             __dmul_rn(quarterJ, (double)o->bJ));
+  const double M = (double)o->M, Ms = (double)o->Ms;
+  o->sumE = __dadd_rn(o->sumE, E); o->sumE2 = __dadd_rn(o->sumE2, __dmul_rn(E, E));
+  o->sumM = __dadd_rn(o->sumM, M); o->sumM2 = __dadd_rn(o->sumM2, __dmul_rn(M, M)); o->sumAbsM = __dadd_rn(o->sumAbsM, fabs(M));
+  o->sumMs = __dadd_rn(o->sumMs, Ms); o->sumMs2 = __dadd_rn(o->sumMs2, __dmul_rn(Ms, Ms)); o->sumAbsMs = __dadd_rn(o->sumAbsMs, fabs(Ms));
+  o->nmeas += 1;
+  if (trace_row) {
+    long long* t = trace_row + 6LL * r;
+    t[0] = o->n2; t[1] = o->bV; t[2] = o->bJ; t[3] = o->M; t[4] = o->Ms; t[5] = o->Q;
+  }
+}
+
+// Full recomputation of (n2, bV, bJ, M, Ms, Q) straight from eq. (3): every site contributes
+// its on-site term and its +x and +y bond, periodic.  out8 must be zeroed before the launch.
+template <int BITS>
+__global__ void __launch_bounds__(256) k_recompute(const void* lat, int L, int logL, long long* out8) {
+  const long long N = (long long)L * L;
+  const int mask = L - 1;
+  long long acc[6] = {0, 0, 0, 0, 0, 0};
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    const int x = (int)(i & mask), y = (int)(i >> logL);
+    const int c = Sites<BITS>::load(lat, i);
+    const int cr = Sites<BITS>::load(lat, ((long long)y << logL) + ((x + 1) & mask));
+    const int cd = Sites<BITS>::load(lat, ((long long)((y + 1) & mask) << logL) + x);
+    const int S = S_of(c), G = sg_of(c);
+    acc[0] += S * S; acc[1] += S * (S_of(cr) + S_of(cd)); acc[2] += G * (sg_of(cr) + sg_of(cd));
+    acc[3] += G; acc[4] += ((x + y) & 1) ? -G : G; acc[5] += S;
+  }
+  __shared__ long long red[6][8];
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    long long v = acc[k];
+    for (int s = 16; s > 0; s >>= 1) v += __shfl_down_sync(0xFFFFFFFFu, v, s);
+    if (lane == 0) red[k][warp] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    long long v = 0;
+    for (int wv = 0; wv < (int)(blockDim.x >> 5); ++wv) v += red[threadIdx.x][wv];
+    atomicAdd((unsigned long long*)&out8[threadIdx.x], (unsigned long long)v);
+  }
+}
+
+// Public byte codes <-> 2-bit packed words (16 sites per word).  n16 = number of words.
+__global__ void k_pack2(const int8_t* codes, uint32_t* words, long long n16) {
+  for (long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x; wi < n16; wi += (long long)gridDim.x * blockDim.x) {
+    const uint4 v = ((const uint4*)codes)[wi];
+    const uint32_t in[4] = {v.x, v.y, v.z, v.w};
+    uint32_t out = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      uint32_t b = in[k] & 0x03030303u;                       // four codes, one per byte
+      b = (b | (b >> 6)) & 0x000F000Fu; b = (b | (b >> 12)) & 0xFFu;  // -> 8 bits
+      out |= b << (8 * k);
+    }
+    words[wi] = out;
+  }
+}
+__global__ void k_unpack2(const uint32_t* words, int8_t* codes, long long n16) {
+  for (long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x; wi < n16; wi += (long long)gridDim.x * blockDim.x) {
+    const uint32_t wd = words[wi];
+    uint32_t out[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      uint32_t b = (wd >> (8 * k)) & 0xFFu;
+      b = (b | (b << 12)) & 0x000F000Fu; b = (b | (b << 6)) & 0x03030303u;
+      out[k] = b;
+    }
+    ((uint4*)codes)[wi] = make_uint4(out[0], out[1], out[2], out[3]);
+  }
+}
+
+}  // namespace ic

@@ -1,0 +1,301 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): lattices bit-exact, exact integers (n2,bV,bJ,M,Ms,Q) bit-exact, fp64 sums within 1e-6
+relative (they are in fact computed with the same operations in the same order, so the tests also check for equality
+where that holds).  Sum S = Q is checked after every run.
+"""
+import ctypes as C
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+import ic_inputs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+NCPU = os.cpu_count() or 1
+S_OF = np.array([0, 0, 1, -1])
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2301_11735_b200 as p
+    return p
+
+
+def oracle_run(codes, delta, V, J, seed, Ts, nsweeps, trace=False, threads=1):
+    """One oracle lattice per replica (replica index = counter field), run in parallel host threads."""
+    lats = [oracle.Lattice(codes[r], delta, V, J, seed, replica=r) for r in range(len(Ts))]
+
+    def go(r):
+        return lats[r].sweep_s1(Ts[r], nsweeps, trace=trace, threads=threads)
+
+    if len(Ts) > 1 and threads == 1:
+        with ThreadPoolExecutor(max_workers=min(NCPU, len(Ts))) as ex:
+            traces = list(ex.map(go, range(len(Ts))))
+    else:
+        traces = [go(r) for r in range(len(Ts))]
+    return lats, traces
+
+
+def check_against_oracle(sim, lats, Ts, rtol=1e-6, exact_sums=True):
+    obs = sim.observables()
+    for r, lat in enumerate(lats):
+        got = sim.state(r)
+        assert np.array_equal(got, lat.code), f"replica {r}: lattice differs at {np.argwhere(got != lat.code)[:5]}"
+        o, ref = obs[r], lat.observables(Ts[r])
+        for k in ("n2", "bV", "bJ", "M", "Ms", "Q", "nmeas"):
+            assert o[k] == ref[k], (r, k, o[k], ref[k])
+        assert int(S_OF[got].sum()) == sim.Q                              # eq. (2)
+        assert np.array_equal(sim.debug_recompute(r), lat.ints())         # incremental == full recomputation
+        for k in ("sumE", "sumE2", "sumM", "sumM2", "sumAbsM", "sumMs", "sumMs2", "sumAbsMs", "C", "chi_u", "chi_s"):
+            if exact_sums and k.startswith("sum"):
+                assert o[k] == ref[k], (r, k, o[k], ref[k])
+            assert abs(o[k] - ref[k]) <= rtol * max(1.0, abs(ref[k])), (r, k, o[k], ref[k])
+
+
+# ------------------------------------------------------------------------------------------------ host logic
+def test_threshold_table_matches_oracle(pkg):
+    sim = pkg.Sim(16, 0.25, 0.5, 1.0, 1.0, seed=1)
+    for (d, V, J) in [(0.5, 1.0, 1.0), (-0.5, 1.0, 2.0), (0.0, 0.5, 1.0), (1.0, 0.25, 1.0), (0.2, 1.0, 1.0)]:
+        s = pkg.Sim(16, 0.25, d, V, J, seed=1)
+        for T in (0.05, 0.1, 0.8, 1.0, 2.0, 3.2, 4.0):
+            tab = s.thresholds(T)
+            k = 0
+            for dn2 in (-2, 0, 2):
+                for dV in range(-16, 17):
+                    for dJ in range(-16, 17):
+                        assert int(tab[k]) == oracle.threshold(d, V, J, dn2, dV, dJ, T), (d, V, J, T, dn2, dV, dJ)
+                        k += 1
+        s.close()
+    sim.close()
+
+
+def test_schedule_matches_oracle(pkg):
+    for L in (4, 16, 64, 1024):
+        sim = pkg.Sim(L, 0.0, 0, 0, 0, seed=1234567890123)
+        for s in list(range(40)) + [10 ** 6, 2 ** 31 - 2]:
+            assert tuple(sim.schedule(s)) == oracle.schedule_params(L, 1234567890123, s)
+        sim.close()
+
+
+def test_stage1_init_matches_oracle(pkg):
+    for (L, n, seed, reps) in [(16, 0.25, 1, 3), (64, 0.1, 2, 2), (64, -0.3, 9, 1), (256, 0.05, 5, 1), (8, 1.0, 3, 1), (8, 0.0, 3, 1)]:
+        for bits in (8, 2):
+            sim = pkg.Sim(L, n, 0.5, 1.0, 1.0, seed=seed, replicas=reps, bits_per_site=bits)
+            Q = sim.Q
+            assert Q == int(np.floor(abs(n) * L * L + 0.5)) * (1 if n >= 0 else -1)
+            for r in range(reps):
+                ref = oracle.init_state(L, L, max(Q, 0), max(-Q, 0), seed, r)
+                got = sim.state(r)
+                assert np.array_equal(got, ref)
+                assert np.array_equal(sim.debug_recompute(r), oracle.recompute(ref))
+                o = sim.observables()[r]
+                assert [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")] == list(oracle.recompute(ref))
+            sim.close()
+    sim = pkg.Sim(64, 0.0, 0.5, 1.0, 1.0, seed=3)
+    sim.init_charges(0, 700, 700)
+    assert np.array_equal(sim.state(0), oracle.init_state(64, 64, 700, 700, 3, 0))
+    with pytest.raises(pkg.IcError):
+        sim.init_charges(0, 10, 9)
+    sim.close()
+
+
+def test_set_state_validation(pkg):
+    sim = pkg.Sim(16, 0.25, 0.5, 1.0, 1.0, seed=1)
+    good = ic_inputs.random_state(16, 64, 0, seed=5)
+    sim.set_state(0, good)
+    before = sim.state(0).copy()
+    bad = good.copy(); bad[3, 3] = 4
+    with pytest.raises(pkg.IcError) as e:
+        sim.set_state(0, bad)
+    assert e.value.code == pkg.IC_ERR_CHARGE
+    wrongq = ic_inputs.random_state(16, 63, 0, seed=5)
+    with pytest.raises(pkg.IcError):
+        sim.set_state(0, wrongq)
+    assert np.array_equal(sim.state(0), before)             # unchanged on error
+    with pytest.raises(pkg.IcError):
+        sim.sweep(0.0, 1)
+    with pytest.raises(pkg.IcError):
+        sim.sweep(1.0, -1)
+    assert sim.sweep_count == 0
+    sim.close()
+
+
+# ------------------------------------------------------------------------------------------------ trajectories
+PARITY_CASES = [
+    # L, bits, replicas, (nplus, nminus), (delta, V, J), Ts, nsweeps
+    (4, 8, 2, (4, 0), (0.5, 1.0, 1.0), [0.6, 2.0], 200),
+    (4, 2, 1, (2, 2), (-0.5, 1.0, 2.0), [1.5], 200),
+    (8, 8, 3, (6, 0), (0.5, 1.0, 1.0), [0.3, 1.0, 4.0], 150),
+    (8, 2, 2, (0, 10), (0.0, 0.5, 1.0), [0.4, 1.0], 150),
+    (16, 8, 4, (64, 0), (0.5, 1.0, 1.0), [0.1, 0.5, 1.0, 4.0], 120),
+    (16, 2, 2, (64, 0), (0.5, 1.0, 1.0), [0.1, 2.0], 120),
+    (32, 8, 2, (100, 100), (-0.5, 1.0, 2.0), [0.8, 1.6], 80),
+    (64, 8, 5, (410, 0), (0.0, 0.5, 1.0), [0.05, 0.5, 1.0, 2.0, 3.2], 60),
+    (64, 2, 3, (410, 0), (0.0, 0.5, 1.0), [0.05, 1.0, 3.2], 60),
+    (128, 8, 2, (2000, 1000), (1.0, 0.25, 1.0), [0.2, 2.0], 40),
+    (256, 8, 1, (0, 0), (0.2, 1.0, 1.0), [1.0], 30),            # no charges: plain Ising with coupling J/4
+    (256, 2, 2, (20000, 20000), (-0.5, 1.0, 2.0), [0.8, 0.3], 30),
+    (512, 8, 1, (13107, 0), (0.2, 1.0, 1.0), [1.0], 12),
+]
+
+
+@pytest.mark.parametrize("L,bits,reps,charges,par,Ts,nsweeps", PARITY_CASES)
+def test_trajectory_parity(pkg, L, bits, reps, charges, par, Ts, nsweeps):
+    nplus, nminus = charges
+    delta, V, J = par
+    seed = 1000 + L + bits
+    n = (nplus - nminus) / (L * L)
+    codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
+    sim = pkg.Sim(L, n, delta, V, J, seed=seed, replicas=reps, bits_per_site=bits)
+    assert sim.Q == nplus - nminus
+    for r in range(reps):
+        sim.set_state(r, codes[r])
+    tr = sim.sweep_trace(Ts, nsweeps)
+    lats, traces = oracle_run(codes, delta, V, J, seed, Ts, nsweeps, trace=True)
+    check_against_oracle(sim, lats, Ts)
+    tr = tr.cpu().numpy()
+    for r in range(reps):
+        assert np.array_equal(tr[:, r, :], traces[r]), f"per-sweep integers differ, replica {r}"
+        assert (tr[:, r, 5] == sim.Q).all()
+    sim.close()
+
+
+def test_call_splitting_and_reset(pkg):
+    """The sweep counter is global: 30 sweeps == 7 + 0 + 23 sweeps; reset zeroes the sums only."""
+    L, seed = 64, 42
+    code = ic_inputs.random_state(L, 300, 110, seed)
+    a = pkg.Sim(L, 190 / L / L, 0.5, 1.0, 1.0, seed=seed); a.set_state(0, code)
+    b = pkg.Sim(L, 190 / L / L, 0.5, 1.0, 1.0, seed=seed); b.set_state(0, code)
+    a.sweep(1.3, 30)
+    b.sweep(1.3, 7); b.sweep(1.3, 0); b.sweep(1.3, 23)
+    assert a.sweep_count == b.sweep_count == 30
+    assert np.array_equal(a.state(0), b.state(0))
+    assert a.observables()[0] == b.observables()[0]
+    lat = oracle.Lattice(code, 0.5, 1.0, 1.0, seed)
+    lat.sweep_s1(1.3, 30)
+    check_against_oracle(a, [lat], [1.3])
+    a.reset_observables(); lat.reset_observables()
+    a.sweep(0.7, 5); lat.sweep_s1(0.7, 5)        # temperature change between calls
+    check_against_oracle(a, [lat], [0.7])
+    assert a.observables()[0]["nmeas"] == 5
+    a.close(); b.close()
+
+
+def test_frozen_and_degenerate_lattices(pkg):
+    L = 32
+    # n = +-1: every pair has q = +-2, nothing can move; E = N (Delta + 2V) exactly
+    for kind, n in (("all_plus", 1.0), ("all_minus", -1.0)):
+        sim = pkg.Sim(L, n, 0.5, 1.0, 1.0, seed=3)
+        assert (sim.state(0) == (2 if n > 0 else 3)).all()
+        sim.sweep(1.0, 6)
+        o = sim.observables()[0]
+        assert (sim.state(0) == (2 if n > 0 else 3)).all()
+        assert o["sumE"] == 6 * L * L * (0.5 + 2 * 1.0)
+        sim.close()
+    for kind in ("neel", "ferro", "stripes"):
+        code = ic_inputs.structured_state(L, kind)
+        for T in (0.02, 50.0):
+            sim = pkg.Sim(L, 0.0, 0.5, 1.0, 1.0, seed=8, bits_per_site=2); sim.set_state(0, code)
+            lat = oracle.Lattice(code, 0.5, 1.0, 1.0, 8)
+            sim.sweep(T, 20); lat.sweep_s1(T, 20)
+            check_against_oracle(sim, [lat], [T])
+            sim.close()
+
+
+def test_config_c1_full_length(pkg):
+    """BASELINE config 1 at full length: L=16, 41 temperatures, 2000 + 10000 sweeps, fp64 observables."""
+    c = ic_inputs.CONFIGS["C1"]
+    L, Ts = c["L"], c["T"]
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=len(Ts), bits_per_site=8)
+    codes = [sim.state(r).copy() for r in range(len(Ts))]       # stage-1 states (checked against the oracle above)
+    for r in range(len(Ts)):
+        assert np.array_equal(codes[r], oracle.init_state(L, L, c["nplus"], 0, c["seed"], r))
+    lats = [oracle.Lattice(codes[r], c["delta"], c["V"], c["J"], c["seed"], replica=r) for r in range(len(Ts))]
+
+    def go(r):
+        lats[r].sweep_s1(Ts[r], c["equil"]); lats[r].reset_observables(); lats[r].sweep_s1(Ts[r], c["sweeps"])
+
+    with ThreadPoolExecutor(max_workers=NCPU) as ex:
+        list(ex.map(go, range(len(Ts))))
+    sim.sweep(Ts, c["equil"]); sim.reset_observables(); sim.sweep(Ts, c["sweeps"])
+    check_against_oracle(sim, lats, Ts)
+    obs = sim.observables()
+    assert all(o["nmeas"] == c["sweeps"] for o in obs)
+    # with the exact constraint the heat capacity stays finite and -> 0 as T -> 0
+    assert 0.0 <= obs[0]["C"] < 0.2
+    sim.close()
+
+
+def test_config_c2_batched_replicas(pkg):
+    """BASELINE config 2: L=64, 64 temperatures as 64 replicas in one launch (reduced sweep count on the oracle side)."""
+    c = ic_inputs.CONFIGS["C2"]
+    L, Ts, nsw = c["L"], c["T"], 400
+    codes = [ic_inputs.random_state(L, c["nplus"], 0, c["seed"], r) for r in range(len(Ts))]
+    for bits in (8, 2):
+        sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=len(Ts), bits_per_site=bits)
+        for r in range(len(Ts)):
+            sim.set_state(r, codes[r])
+        sim.sweep(Ts, nsw)
+        if bits == 8:
+            lats, _ = oracle_run(codes, c["delta"], c["V"], c["J"], c["seed"], Ts, nsw)
+        check_against_oracle(sim, lats, Ts)
+        sim.close()
+
+
+def test_config_c3_packed_l1024(pkg):
+    """BASELINE config 3: L=1024, neutral with both charge signs at density 0.3, 2-bit packed state."""
+    c = ic_inputs.CONFIGS["C3"]
+    L, nsw = c["L"], 24
+    code = ic_inputs.random_state(L, c["nplus"], c["nminus"], c["seed"])
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=2); sim.set_state(0, code)
+    lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
+    sim.sweep(c["T"], nsw); lat.sweep_s1(c["T"][0], nsw, threads=NCPU)
+    check_against_oracle(sim, [lat], c["T"])
+    sim.close()
+
+
+def test_config_c4_trace_l4096(pkg):
+    """BASELINE config 4 (2 of its 16 replicas on the oracle side): per-sweep integers via ic_sweep_trace."""
+    c = ic_inputs.CONFIGS["C4"]
+    L, nsw = c["L"], 4
+    Ts = [c["T"][0], c["T"][15]]
+    codes = [ic_inputs.random_state(L, c["nplus"], 0, c["seed"], r) for r in range(2)]
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=2, bits_per_site=8)
+    for r in range(2):
+        sim.set_state(r, codes[r])
+    tr = sim.sweep_trace(Ts, nsw).cpu().numpy()
+    lats = [oracle.Lattice(codes[r], c["delta"], c["V"], c["J"], c["seed"], replica=r) for r in range(2)]
+    for r in range(2):
+        t = lats[r].sweep_s1(Ts[r], nsw, trace=True, threads=NCPU)
+        assert np.array_equal(tr[:, r, :], t)
+    check_against_oracle(sim, lats, Ts)
+    sim.close()
+
+
+def test_config_c5_full_size_sampled(pkg):
+    """BASELINE config 5 at its full size (L=16384, the launch configuration bench.py times): two sweeps (one FAR, one
+    NEAR) against the multi-threaded oracle, whole lattice compared; then invariants after more sweeps."""
+    c = ic_inputs.CONFIGS["C5"]
+    L = c["L"]
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=8)
+    code = sim.state(0).copy()
+    assert int(S_OF[code].sum()) == sim.Q == c["nplus"]
+    lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
+    sim.sweep(c["T"], 2); lat.sweep_s1(c["T"][0], 2, threads=NCPU)
+    got = sim.state(0)
+    assert np.array_equal(got, lat.code)
+    o = sim.observables()[0]; ref = lat.observables(c["T"][0])
+    for k in ("n2", "bV", "bJ", "M", "Ms", "Q", "sumE", "sumE2", "sumM2", "sumMs2"):
+        assert o[k] == ref[k], (k, o[k], ref[k])
+    sim.sweep(c["T"], 6)
+    assert int(S_OF[sim.state(0)].sum()) == sim.Q
+    o = sim.observables()[0]
+    assert list(sim.debug_recompute(0)) == [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    sim.close()
