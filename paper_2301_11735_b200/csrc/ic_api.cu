@@ -15,20 +15,21 @@
 #include "../../include/ic.h"
 #include "ic_common.cuh"
 #include "ic_kernels_ref.cuh"
+#include "ic_kernels_p16.cuh"
 
 using namespace ic;
 
 struct ic_ctx {
-  int L, logL, replicas, bits, variant;
+  int L, logL, replicas, bits, variant, layout;
   long long N, Q;
   double n, delta, V, J;
   uint64_t seed, sweep;
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint32_t* d_thr; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
   // host (pinned)
-  uint32_t* h_thr; ReplicaObs* h_obs;
+  uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
   std::vector<double>* lastT; bool have_T;
   long long launches;
@@ -56,7 +57,8 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   if (!valid_dims(L, replicas, bits)) return 0;
   size_t b = 0;
   b += align256(lattice_bytes(L, bits)) * (size_t)replicas;       // lattices
-  b += align256((size_t)replicas * THR_STRIDE * sizeof(uint32_t)); // thresholds
+  b += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));    // class tables (threshold, packed deltas)
+  b += align256(2 * DESC_ENTRIES * sizeof(uint2));                 // move descriptors, FAR and NEAR
   b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
   b += 256;                                                        // scratch for ic_debug_recompute
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
@@ -78,6 +80,59 @@ static void build_thresholds(const ic_ctx* c, double T, uint32_t* out) {
   for (int a = -1; a <= 1; ++a)
     for (int v = -16; v <= 16; ++v)
       for (int j = -16; j <= 16; ++j) out[class_index(2 * a, v, j)] = threshold29(c->delta, c->V, qJ, 2 * a, v, j, T);
+}
+// Device form of the class table: (8*t29 - 1, packed (dn2, dV, dJ)); w <= 8*t29 - 1  <=>  (w >> 3) < t29.
+static void build_class_table(const ic_ctx* c, double T, uint2* out) {
+  uint32_t t29[N_CLASSES];
+  build_thresholds(c, T, t29);
+  for (int a = -1; a <= 1; ++a)
+    for (int v = -16; v <= 16; ++v)
+      for (int j = -16; j <= 16; ++j) {
+        const int k = class_index(2 * a, v, j);
+        out[k].x = 8u * t29[k] - 1u;
+        out[k].y = (uint32_t)pack_delta(2 * a, v, j);
+      }
+  for (int k = N_CLASSES; k < THR_STRIDE; ++k) { out[k].x = 0u; out[k].y = 0u; }
+}
+
+// The table of two-site configurations in the paper's listing order, as move descriptors for the
+// tiled kernels.  Entry [key*8 + r], key = fa | fb<<1 | ga<<3 | gb<<4 in the (f,g) site encoding of LAY_P16:
+//   x = int8 x 4 (cFa, cGa, cFb, cGb): class index = K + cFa*Fa + cGa*Ga + cFb*Fb + cGb*Gb, where the neighbour sums are
+//       sum S = F+G-4, sum sigma = F-G, i.e. cF = 33*dS + dsig, cG = 33*dS - dsig (the -4 cancels: dS_a + dS_b = 0);
+//   y = 8*K | (xor of the site bytes: a at bits 0,3, b at bits 1,4) << 16 | (dM & 15 | (dD & 15) << 4) << 24,
+//       K = class_index(E_Delta, adj*dS_a*dS_b, adj*dsig_a*dsig_b)  (eq. 4 for adj = 0, eq. 5 for adj = 1),
+//       dM = dsig_a + dsig_b, dD = dsig_a - dsig_b.
+// Null proposals (q = +-2, r >= 6 for q = 0, the current configuration) have x = 0 and no change: class (0,0,0).
+static void build_descriptors(int adj, uint2* out) {
+  static const int Q0[6][2] = {{2, 3}, {3, 2}, {0, 0}, {1, 1}, {0, 1}, {1, 0}};
+  for (int key = 0; key < 28; ++key)
+    for (int r = 0; r < 8; ++r) {
+      uint2 d; d.x = 0u; d.y = 8u * (uint32_t)class_index(0, 0, 0);
+      const int ea = (key & 1) | (key & 8), eb = ((key >> 1) & 1) | ((key >> 1) & 8);
+      const bool valid = (key & ~0x1B) == 0;
+      if (valid) {
+        const int ca = code_of_e(ea), cb = code_of_e(eb);
+        const int q = S_of(ca) + S_of(cb);
+        int na = ca, nb = cb;
+        if (q == 0) { if (r < 6) { na = Q0[r][0]; nb = Q0[r][1]; } }
+        else if (q == 1 || q == -1) {
+          const int C = q > 0 ? 2 : 3;
+          switch (r & 3) { case 0: na = C; nb = 0; break; case 1: na = C; nb = 1; break; case 2: na = 0; nb = C; break; default: na = 1; nb = C; }
+        }
+        if (na != ca || nb != cb) {
+          const int dSa = S_of(na) - S_of(ca), dSb = S_of(nb) - S_of(cb), dGa = sg_of(na) - sg_of(ca), dGb = sg_of(nb) - sg_of(cb);
+          const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
+          const int K = class_index(e_d, adj * dSa * dSb, adj * dGa * dGb);
+          const int cf[4] = {33 * dSa + dGa, 33 * dSa - dGa, 33 * dSb + dGb, 33 * dSb - dGb};
+          d.x = 0u;
+          for (int k = 0; k < 4; ++k) d.x |= ((uint32_t)(cf[k] & 0xFF)) << (8 * k);
+          const int xa = ea ^ e_of_code(na), xb = eb ^ e_of_code(nb);
+          const int dM = dGa + dGb, dD = dGa - dGb;
+          d.y = 8u * (uint32_t)K | ((uint32_t)(xa | (xb << 1)) << 16) | ((uint32_t)((dM & 15) | ((dD & 15) << 4)) << 24);
+        }
+      }
+      out[key * 8 + r] = d;
+    }
 }
 
 // U4: parameters of sweep s, from Philox(ctr = (0, 0, s, TAG_SCHED), key = seed); the same for all replicas.
@@ -135,10 +190,11 @@ __global__ void k_store_ints(ReplicaObs* o, const long long* s8) {
 
 static int recompute_into_scratch(ic_ctx* c, int replica) {
   IC_CUDA(cudaMemsetAsync(c->d_scratch8, 0, 64, c->stream));
-  const void* lat = c->lattice + (long long)replica * c->lat_stride;
+  const LatView lat{c->lattice + (long long)replica * c->lat_stride, c->L, c->logL};
   const int blocks = (int)std::min<long long>((c->N + 255) / 256, 148 * 8);
-  if (c->bits == 8) k_recompute<8><<<blocks, 256, 0, c->stream>>>(lat, c->L, c->logL, c->d_scratch8);
-  else k_recompute<2><<<blocks, 256, 0, c->stream>>>(lat, c->L, c->logL, c->d_scratch8);
+  if (c->layout == LAY_ROW8) k_recompute<LAY_ROW8><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
+  else if (c->layout == LAY_ROW2) k_recompute<LAY_ROW2><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
+  else k_recompute<LAY_P16><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
@@ -147,13 +203,14 @@ static int recompute_into_scratch(ic_ctx* c, int replica) {
 // Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.
 static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
   char* lat = c->lattice + (long long)replica * c->lat_stride;
-  if (c->bits == 8) {
+  if (c->layout == LAY_ROW8) {
     IC_CUDA(cudaMemcpyAsync(lat, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
   } else {
     IC_CUDA(cudaMemcpyAsync(c->d_stage, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
     const long long n16 = c->N / 16;
-    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 8);
-    k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 16);
+    if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
+    else k_codes_to_p16<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint8_t*)lat, c->logL);
     c->launches++;
     IC_CUDA(cudaGetLastError());
   }
@@ -178,25 +235,34 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   if (!c) return IC_ERR_NULL;
   c->L = L; c->logL = 0; while ((1 << c->logL) < L) c->logL++;
   c->replicas = replicas; c->bits = bits; c->variant = 0;
+  c->layout = bits == 2 ? LAY_ROW2 : (L >= 64 ? LAY_P16 : LAY_ROW8);
   c->N = (long long)L * L; c->Q = std::llround(n * (double)c->N);
   c->n = n; c->delta = delta; c->V = V; c->J = J; c->seed = seed; c->sweep = 0;
   c->stream = (cudaStream_t)cuda_stream;
   c->launches = 0; c->have_T = false; c->lastT = new std::vector<double>((size_t)replicas, 0.0);
   char* p = (char*)d_workspace;
   c->lattice = p; c->lat_stride = (long long)align256(lattice_bytes(L, bits)); p += (size_t)c->lat_stride * replicas;
-  c->d_thr = (uint32_t*)p; p += align256((size_t)replicas * THR_STRIDE * sizeof(uint32_t));
+  c->d_thr = (uint2*)p; p += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));
+  c->d_desc = (uint2*)p; p += align256(2 * DESC_ENTRIES * sizeof(uint2));
   c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
   c->d_scratch8 = (long long*)p; p += 256;
   c->d_stage = (int8_t*)p;
   c->h_thr = nullptr; c->h_obs = nullptr; c->thr_copied = nullptr;
 
   auto fail = [&](int rc) { ic_destroy(c); return rc; };
-  if (cudaMallocHost((void**)&c->h_thr, (size_t)replicas * THR_STRIDE * sizeof(uint32_t)) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost(thresholds)"));
+  if (cudaMallocHost((void**)&c->h_thr, (size_t)replicas * THR_STRIDE * sizeof(uint2)) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost(thresholds)"));
   if (cudaMallocHost((void**)&c->h_obs, (size_t)replicas * sizeof(ReplicaObs)) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost(observables)"));
   if (cudaEventCreateWithFlags(&c->thr_copied, cudaEventDisableTiming) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaEventCreate"));
-  memset(c->h_thr, 0, (size_t)replicas * THR_STRIDE * sizeof(uint32_t));
+  memset(c->h_thr, 0, (size_t)replicas * THR_STRIDE * sizeof(uint2));
   cudaError_t e = cudaMemsetAsync(c->d_obs, 0, (size_t)replicas * sizeof(ReplicaObs), c->stream);
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaMemsetAsync(observables)"));
+  {
+    std::vector<uint2> desc(2 * DESC_ENTRIES);
+    build_descriptors(0, desc.data()); build_descriptors(1, desc.data() + DESC_ENTRIES);
+    e = cudaMemcpyAsync(c->d_desc, desc.data(), desc.size() * sizeof(uint2), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the move descriptors"));
+  }
 
   // stage 1 for every replica
   std::vector<int8_t> codes((size_t)c->N);
@@ -260,12 +326,13 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
   if (!c || !h_out) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
   const char* lat = c->lattice + (long long)replica * c->lat_stride;
-  if (c->bits == 8) {
+  if (c->layout == LAY_ROW8) {
     IC_CUDA(cudaMemcpyAsync(h_out, lat, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
   } else {
     const long long n16 = c->N / 16;
-    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 8);
-    k_unpack2<<<blocks, 256, 0, c->stream>>>((const uint32_t*)lat, c->d_stage, n16);
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 16);
+    if (c->layout == LAY_ROW2) k_unpack2<<<blocks, 256, 0, c->stream>>>((const uint32_t*)lat, c->d_stage, n16);
+    else k_p16_to_codes<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
     c->launches++;
     IC_CUDA(cudaGetLastError());
     IC_CUDA(cudaMemcpyAsync(h_out, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
@@ -277,8 +344,33 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
 static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
   const long long npairs = c->N / 4;
   dim3 grid((unsigned)((npairs + 255) / 256), (unsigned)c->replicas);
-  if (c->bits == 8) k_ref_phase<8><<<grid, 256, 0, c->stream>>>(a);
-  else k_ref_phase<2><<<grid, 256, 0, c->stream>>>(a);
+  if (c->layout == LAY_ROW8) k_ref_phase<LAY_ROW8><<<grid, 256, 0, c->stream>>>(a);
+  else if (c->layout == LAY_ROW2) k_ref_phase<LAY_ROW2><<<grid, 256, 0, c->stream>>>(a);
+  else k_ref_phase<LAY_P16><<<grid, 256, 0, c->stream>>>(a);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
+// Tiled kernels on LAY_P16: one item (32 pair updates) per thread, persistent blocks over the items of a replica.
+static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
+  const long long n_items = c->N / 128;
+  const long long nb = (n_items + P16_THREADS - 1) / P16_THREADS;
+  const long long cap = std::max<long long>(1, (148LL * 6 + c->replicas - 1) / c->replicas);
+  dim3 grid((unsigned)std::min(nb, cap), (unsigned)c->replicas);
+  if (a.type == 0) {
+    a.desc = c->d_desc;
+    switch (((a.p1 >> 2) & 15) >> 2) {
+      case 0: k_p16_phase<PH_FAR, 0><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
+      case 1: k_p16_phase<PH_FAR, 1><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
+      case 2: k_p16_phase<PH_FAR, 2><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
+      default: k_p16_phase<PH_FAR, 3><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
+    }
+  } else {
+    a.desc = c->d_desc + DESC_ENTRIES;
+    if (a.p1 == 0) k_p16_phase<PH_NEAR_H, 0><<<grid, P16_THREADS, 0, c->stream>>>(a);
+    else k_p16_phase<PH_NEAR_V, 0><<<grid, P16_THREADS, 0, c->stream>>>(a);
+  }
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
@@ -298,16 +390,16 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     IC_CUDA(cudaEventSynchronize(c->thr_copied));   // the previous upload has left the pinned buffer
     for (int r = 0; r < c->replicas; ++r) {
       if (c->have_T && (*c->lastT)[r] == h_T[r]) continue;
-      build_thresholds(c, h_T[r], c->h_thr + (size_t)r * THR_STRIDE);
+      build_class_table(c, h_T[r], c->h_thr + (size_t)r * THR_STRIDE);
       (*c->lastT)[r] = h_T[r];
     }
-    IC_CUDA(cudaMemcpyAsync(c->d_thr, c->h_thr, (size_t)c->replicas * THR_STRIDE * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
+    IC_CUDA(cudaMemcpyAsync(c->d_thr, c->h_thr, (size_t)c->replicas * THR_STRIDE * sizeof(uint2), cudaMemcpyHostToDevice, c->stream));
     IC_CUDA(cudaEventRecord(c->thr_copied, c->stream));
     c->have_T = true;
   }
 
   PhaseArgs a;
-  a.lattice = c->lattice; a.thr = c->d_thr; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
   a.L = c->L; a.logL = c->logL; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const double qJ = 0.25 * c->J;
   for (int64_t s = 0; s < nsweeps; ++s) {
@@ -316,7 +408,8 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     a.type = par[0]; a.p1 = par[1]; a.p2 = par[2];
     for (int phase = 0; phase < 2; ++phase) {
       a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
-      int rc = launch_phase_ref(c, a);
+      const bool tiled = c->layout == LAY_P16 && c->variant != 1;
+      int rc = tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
       if (rc != IC_OK) return rc;
     }
     k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ,
@@ -407,7 +500,8 @@ extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->lau
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {
   if (!c) return IC_ERR_NULL;
-  if (variant < 0 || variant > 1) return IC_ERR_PARAM;
+  if (variant < 0 || variant > 2) return IC_ERR_PARAM;
+  if (variant == 2 && c->layout != LAY_P16) return IC_ERR_PARAM;
   c->variant = variant;
   return IC_OK;
 }

@@ -47,9 +47,52 @@ IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, ui
 IC_HD int S_of(int c) { return (c & 2) ? 1 - 2 * (c & 1) : 0; }
 IC_HD int sg_of(int c) { return (c & 2) ? 0 : 1 - 2 * (c & 1); }
 
+// ---------------------------------------------------------------------------------------------------
+// Lattice layouts in device memory.
+//   ROW8  one byte per site, public code, row-major [y][x]                       (8 bits/site, L < 64)
+//   ROW2  2 bits per site, public code, 16 sites per 32-bit word, row-major       (2 bits/site)
+//   P16   one byte per site in 16 planes [y&3][x&3][y>>2][x>>2]; byte e = f | g<<3 with
+//         (f,g) = sigma+ (1,0), sigma- (0,1), S+ (1,1), S- (0,0), so that the byte-wise sum of the four
+//         neighbour bytes is F | G<<3 with  sum S = F+G-4,  sum sigma = F-G        (8 bits/site, L >= 64)
+// Every phase of schedule S1 updates whole planes of P16, so the tiled kernels work on dense 16-byte vectors.
+// ---------------------------------------------------------------------------------------------------
+enum Layout : int { LAY_ROW8 = 0, LAY_ROW2 = 1, LAY_P16 = 2 };
+
+IC_HD int e_of_code(int c) { return (~c & 1) | (((c ^ (c >> 1)) & 1) << 3); }
+IC_HD int code_of_e(int e) { int b0 = ~e & 1; return b0 | ((((e >> 3) ^ b0) & 1) << 1); }
+
+struct LatView {              // one replica
+  char* base;
+  int L, logL;
+};
+
+template <int LAY>
+struct Sites {
+  static __device__ __forceinline__ long long p16_offset(const LatView& v, int x, int y) {
+    const int lw = v.logL - 2;
+    return ((((long long)((y & 3) * 4 + (x & 3)) << lw) + (y >> 2)) << lw) + (x >> 2);
+  }
+  static __device__ __forceinline__ int load(const LatView& v, int x, int y) {
+    if (LAY == LAY_P16) return code_of_e(((const uint8_t*)v.base)[p16_offset(v, x, y)]);
+    const long long i = ((long long)y << v.logL) + x;
+    if (LAY == LAY_ROW8) return ((const int8_t*)v.base)[i];
+    return (((const uint32_t*)v.base)[i >> 4] >> (2 * (int)(i & 15))) & 3;
+  }
+  // Sites written in one phase are distinct; with ROW2 several threads share a word: xor the change in.
+  static __device__ __forceinline__ void store(const LatView& v, int x, int y, int oldc, int newc) {
+    if (LAY == LAY_P16) { ((uint8_t*)v.base)[p16_offset(v, x, y)] = (uint8_t)e_of_code(newc); return; }
+    const long long i = ((long long)y << v.logL) + x;
+    if (LAY == LAY_ROW8) ((int8_t*)v.base)[i] = (int8_t)newc;
+    else atomicXor(&((uint32_t*)v.base)[i >> 4], (uint32_t)(oldc ^ newc) << (2 * (int)(i & 15)));
+  }
+};
+
 // Acceptance class of a move (E_Delta, E_V, E_J): dn2 in {-2,0,2}, dV, dJ in [-16,16].
 constexpr int N_CLASSES = 3 * 33 * 33;   // 3267
-constexpr int THR_STRIDE = 3328;         // table stride per replica (multiple of 64 words)
+constexpr int THR_STRIDE = 3328;         // table entries per replica (multiple of 64)
+// Device table entry of a class: x = 8*t29 - 1 (the move is accepted iff w <= x, which is (w >> 3) < t29),
+// y = packed (dn2, dV, dJ) = dJ + (dV << 11) + (dn2 << 22) for the per-thread observable accumulator.
+IC_HD int pack_delta(int dn2, int dV, int dJ) { return dJ + dV * 2048 + dn2 * 4194304; }
 IC_HD int class_index(int dn2, int dV, int dJ) { return ((dn2 / 2 + 1) * 33 + (dV + 16)) * 33 + (dJ + 16); }
 
 // Per-replica record in device memory: exact integers, then the fp64 sums of U5.
@@ -64,7 +107,8 @@ static_assert(sizeof(ReplicaObs) == 128, "ReplicaObs layout");
 // (precedent: identical maps for all lattice copies).
 struct PhaseArgs {
   void* lattice;                 // [replicas][lat_stride bytes]
-  const uint32_t* thr;           // [replicas][THR_STRIDE] thresholds t29
+  const uint2* thr;              // [replicas][THR_STRIDE] (8*t29-1, packed deltas)
+  const uint2* desc;             // move descriptors of this sweep type (tiled kernels), [28*8]
   ReplicaObs* obs;               // [replicas]
   long long lat_stride;          // bytes per replica
   int L, logL;

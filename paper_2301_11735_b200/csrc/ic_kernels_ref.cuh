@@ -1,27 +1,13 @@
 // ic_kernels_ref.cuh -- variant 1: one thread per coupled pair, lattice in global memory.
 //
 // The plain CUDA statement of the pair update (sec. 3.1) under schedule S1 (U4).
-// It runs any power-of-two L >= 4 at 8 or 2 bits per site and is the in-library cross-check for the tiled
-// and resident kernels; it is also what tiny lattices (L < 16) use.  Each thread recomputes the Philox block
+// It runs any power-of-two L >= 4 in every layout (ROW8, ROW2, P16) and is the in-library cross-check for the
+// tiled kernels; it is also what small lattices (L < 64) and 2-bit states use.  Each thread recomputes the Philox block
 // of its group of four pairs and keeps one word.
 #pragma once
 #include "ic_common.cuh"
 
 namespace ic {
-
-template <int BITS>
-struct Sites {
-  // BITS == 8: one byte per site.  BITS == 2: 16 sites per 32-bit word, site i at bits 2(i&15) of word i>>4.
-  static __device__ __forceinline__ int load(const void* base, long long i) {
-    if (BITS == 8) return ((const int8_t*)base)[i];
-    return (((const uint32_t*)base)[i >> 4] >> (2 * (int)(i & 15))) & 3;
-  }
-  // Sites written in one phase are distinct, but with BITS == 2 several threads share a word: xor the change in.
-  static __device__ __forceinline__ void store(void* base, long long i, int oldc, int newc) {
-    if (BITS == 8) ((int8_t*)base)[i] = (int8_t)newc;
-    else atomicXor(&((uint32_t*)base)[i >> 4], (uint32_t)(oldc ^ newc) << (2 * (int)(i & 15)));
-  }
-};
 
 // Sum of five per-thread integers over the block, then one atomicAdd per value into the replica record.
 __device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV, int dJ, int dM, int dMs) {
@@ -46,13 +32,13 @@ __device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV,
   }
 }
 
-template <int BITS>
+template <int LAY>
 __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
   const int L = A.L, logL = A.logL, mask = L - 1;
   const int r = blockIdx.y;
   const long long npairs = ((long long)L * L) >> 2;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  void* lat = (char*)A.lattice + (long long)r * A.lat_stride;
+  const LatView lat{(char*)A.lattice + (long long)r * A.lat_stride, L, logL};
   int dn2 = 0, dV = 0, dJ = 0, dM = 0, dMs = 0;
   if (t < npairs) {
     // --- which pair (schedule S1) and which random word ---------------------------------------------
@@ -74,8 +60,7 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
     uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
 
     // --- proposal: same pair charge q, configuration r of the paper's list ----------
-    const long long ia = ((long long)ya << logL) + xa, ib = ((long long)yb << logL) + xb;
-    const int ca = Sites<BITS>::load(lat, ia), cb = Sites<BITS>::load(lat, ib);
+    const int ca = Sites<LAY>::load(lat, xa, ya), cb = Sites<LAY>::load(lat, xb, yb);
     const int q = S_of(ca) + S_of(cb);
     const int rr = (int)(w & 7u);
     int na = ca, nb = cb;
@@ -102,11 +87,11 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
     if (na != ca || nb != cb) {
       // --- neighbour sums over the four slots of a and of b, current lattice ----------
       const int xl = (xa - 1) & mask, xr = (xa + 1) & mask, yu = (ya - 1) & mask, yd = (ya + 1) & mask;
-      const int c1 = Sites<BITS>::load(lat, ((long long)ya << logL) + xl), c2 = Sites<BITS>::load(lat, ((long long)ya << logL) + xr);
-      const int c3 = Sites<BITS>::load(lat, ((long long)yu << logL) + xa), c4 = Sites<BITS>::load(lat, ((long long)yd << logL) + xa);
+      const int c1 = Sites<LAY>::load(lat, xl, ya), c2 = Sites<LAY>::load(lat, xr, ya);
+      const int c3 = Sites<LAY>::load(lat, xa, yu), c4 = Sites<LAY>::load(lat, xa, yd);
       const int xl2 = (xb - 1) & mask, xr2 = (xb + 1) & mask, yu2 = (yb - 1) & mask, yd2 = (yb + 1) & mask;
-      const int e1 = Sites<BITS>::load(lat, ((long long)yb << logL) + xl2), e2 = Sites<BITS>::load(lat, ((long long)yb << logL) + xr2);
-      const int e3 = Sites<BITS>::load(lat, ((long long)yu2 << logL) + xb), e4 = Sites<BITS>::load(lat, ((long long)yd2 << logL) + xb);
+      const int e1 = Sites<LAY>::load(lat, xl2, yb), e2 = Sites<LAY>::load(lat, xr2, yb);
+      const int e3 = Sites<LAY>::load(lat, xb, yu2), e4 = Sites<LAY>::load(lat, xb, yd2);
       const int nSa = S_of(c1) + S_of(c2) + S_of(c3) + S_of(c4), nGa = sg_of(c1) + sg_of(c2) + sg_of(c3) + sg_of(c4);
       const int nSb = S_of(e1) + S_of(e2) + S_of(e3) + S_of(e4), nGb = sg_of(e1) + sg_of(e2) + sg_of(e3) + sg_of(e4);
       // --- dE class: eq. (4) distant / eq. (5) neighbouring sites, spin term as in DESIGN.md G1 ------
@@ -115,10 +100,10 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
       const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
       const int e_v = dSa * nSa + dSb * nSb + adj * dSa * dSb;
       const int e_j = dGa * nGa + dGb * nGb + adj * dGa * dGb;
-      const uint32_t t29 = __ldg(&A.thr[(long long)r * THR_STRIDE + class_index(e_d, e_v, e_j)]);
-      if ((w >> 3) < t29) {            // Metropolis min(1, exp(-dE/T)) as an integer compare
-        Sites<BITS>::store(lat, ia, ca, na);
-        Sites<BITS>::store(lat, ib, cb, nb);
+      const uint32_t t8 = __ldg(&A.thr[(long long)r * THR_STRIDE + class_index(e_d, e_v, e_j)]).x;
+      if (w <= t8) {                   // Metropolis min(1, exp(-dE/T)): (w >> 3) < t29, t8 = 8 t29 - 1
+        Sites<LAY>::store(lat, xa, ya, ca, na);
+        Sites<LAY>::store(lat, xb, yb, cb, nb);
         dn2 = e_d; dV = e_v; dJ = e_j; dM = dGa + dGb;
         dMs = (((xa + ya) & 1) ? -dGa : dGa) + (((xb + yb) & 1) ? -dGb : dGb);
       }
@@ -148,16 +133,17 @@ __global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, do
 
 // Full recomputation of (n2, bV, bJ, M, Ms, Q) straight from eq. (3): every site contributes
 // its on-site term and its +x and +y bond, periodic.  out8 must be zeroed before the launch.
-template <int BITS>
-__global__ void __launch_bounds__(256) k_recompute(const void* lat, int L, int logL, long long* out8) {
+template <int LAY>
+__global__ void __launch_bounds__(256) k_recompute(LatView lat, long long* out8) {
+  const int L = lat.L, logL = lat.logL;
   const long long N = (long long)L * L;
   const int mask = L - 1;
   long long acc[6] = {0, 0, 0, 0, 0, 0};
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
     const int x = (int)(i & mask), y = (int)(i >> logL);
-    const int c = Sites<BITS>::load(lat, i);
-    const int cr = Sites<BITS>::load(lat, ((long long)y << logL) + ((x + 1) & mask));
-    const int cd = Sites<BITS>::load(lat, ((long long)((y + 1) & mask) << logL) + x);
+    const int c = Sites<LAY>::load(lat, x, y);
+    const int cr = Sites<LAY>::load(lat, (x + 1) & mask, y);
+    const int cd = Sites<LAY>::load(lat, x, (y + 1) & mask);
     const int S = S_of(c), G = sg_of(c);
     acc[0] += S * S; acc[1] += S * (S_of(cr) + S_of(cd)); acc[2] += G * (sg_of(cr) + sg_of(cd));
     acc[3] += G; acc[4] += ((x + y) & 1) ? -G : G; acc[5] += S;

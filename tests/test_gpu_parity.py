@@ -299,3 +299,34 @@ def test_config_c5_full_size_sampled(pkg):
     o = sim.observables()[0]
     assert list(sim.debug_recompute(0)) == [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     sim.close()
+
+
+# ------------------------------------------------------------------------------------------------ kernel variants
+@pytest.mark.parametrize("L,reps,nsweeps", [(64, 3, 64), (128, 2, 64), (256, 2, 48), (1024, 1, 40), (4096, 1, 12)])
+def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps):
+    """Variant 2 (tiled, 16-plane layout) against variant 1 (one thread per pair) on the same device memory layout,
+    sweep by sweep so that many (mx, my) masks, both domino orientations and all four offsets are exercised; the
+    reference kernels are themselves compared with the oracle above and (at L <= 256) here."""
+    seed = 4242 + L
+    nplus, nminus = L * L // 10, L * L // 20
+    n = (nplus - nminus) / (L * L)
+    Ts = [0.4, 1.1, 2.5][:reps]
+    codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
+    a = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); a.set_variant(2)
+    b = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); b.set_variant(1)
+    for r in range(reps):
+        a.set_state(r, codes[r]); b.set_state(r, codes[r])
+    seen = set()
+    for s in range(nsweeps):
+        seen.add(a.schedule(s)[:2] if a.schedule(s)[0] else (0, (a.schedule(s)[1] >> 2) & 15))
+        a.sweep(Ts, 1); b.sweep(Ts, 1)
+        oa, ob = a.observables(), b.observables()
+        for r in range(reps):
+            assert oa[r] == ob[r], (s, r, a.schedule(s))
+        if s % 8 == 7 or s == nsweeps - 1:
+            for r in range(reps):
+                assert np.array_equal(a.state(r), b.state(r)), (s, r, a.schedule(s))
+    if L <= 256:
+        lats, _ = oracle_run(codes, 0.3, 1.0, 1.5, seed, Ts, nsweeps)
+        check_against_oracle(a, lats, Ts)
+    a.close(); b.close()
