@@ -16,6 +16,7 @@
 #include "ic_common.cuh"
 #include "ic_kernels_ref.cuh"
 #include "ic_kernels_p16.cuh"
+#include "ic_kernels_staged.cuh"
 
 using namespace ic;
 
@@ -27,12 +28,13 @@ struct ic_ctx {
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint2* d_thr; uint2* d_desc; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; uint4* d_desc16; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
   // host (pinned)
   uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
   std::vector<double>* lastT; bool have_T;
   long long launches;
+  int sm_count;
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -59,6 +61,7 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   b += align256(lattice_bytes(L, bits)) * (size_t)replicas;       // lattices
   b += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));    // class tables (threshold, packed deltas)
   b += align256(2 * DESC_ENTRIES * sizeof(uint2));                 // move descriptors, FAR and NEAR
+  b += align256(ST_DESC_BYTES);                                    // 16-byte move descriptors (staged kernels)
   b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
   b += 256;                                                        // scratch for ic_debug_recompute
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
@@ -133,6 +136,22 @@ static void build_descriptors(int adj, uint2* out) {
       }
       out[key * 8 + r] = d;
     }
+}
+
+// The same table for the staged kernels: 16-byte entries at [key][adj][r] (key*256 + adj*128 + r*16 bytes):
+//   x = the four int8 coefficients, y = 8*K (byte offset of the class base in the class table),
+//   z = xor of the site bytes | (dM & 15 | (dD & 15) << 4) << 8, w = 0.
+static void build_descriptors16(uint4* out) {
+  std::vector<uint2> d8(DESC_ENTRIES);
+  for (int adj = 0; adj < 2; ++adj) {
+    build_descriptors(adj, d8.data());
+    for (int key = 0; key < 28; ++key)
+      for (int r = 0; r < 8; ++r) {
+        const uint2 d = d8[key * 8 + r];
+        uint4 q; q.x = d.x; q.y = d.y & 0x7FFFu; q.z = ((d.y >> 16) & 0xFFu) | (((d.y >> 24) & 0xFFu) << 8); q.w = 0u;
+        out[key * 16 + adj * 8 + r] = q;
+      }
+  }
 }
 
 // U4: parameters of sweep s, from Philox(ctr = (0, 0, s, TAG_SCHED), key = seed); the same for all replicas.
@@ -244,6 +263,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   c->lattice = p; c->lat_stride = (long long)align256(lattice_bytes(L, bits)); p += (size_t)c->lat_stride * replicas;
   c->d_thr = (uint2*)p; p += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));
   c->d_desc = (uint2*)p; p += align256(2 * DESC_ENTRIES * sizeof(uint2));
+  c->d_desc16 = (uint4*)p; p += align256(ST_DESC_BYTES);
   c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
   c->d_scratch8 = (long long*)p; p += 256;
   c->d_stage = (int8_t*)p;
@@ -262,6 +282,15 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
     e = cudaMemcpyAsync(c->d_desc, desc.data(), desc.size() * sizeof(uint2), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the move descriptors"));
+    std::vector<uint4> desc16(ST_DESC_BYTES / 16);
+    build_descriptors16(desc16.data());
+    e = cudaMemcpyAsync(c->d_desc16, desc16.data(), ST_DESC_BYTES, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the 16-byte move descriptors"));
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+      return fail(cuda_fail(cudaGetLastError(), "cudaDeviceGetAttribute(multiProcessorCount)"));
+    c->sm_count = sms;
   }
 
   // stage 1 for every replica
@@ -376,6 +405,41 @@ static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
   return IC_OK;
 }
 
+// Staged kernels on LAY_P16, L >= 2048: one persistent block per SM, TMA-staged regions (ic_kernels_staged.cuh).
+template <int TYPE, int CW>
+static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
+  using C = StagedCfg<TYPE>;
+  static bool configured = false;   // per instantiation
+  if (!configured) {
+    IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    configured = true;
+  }
+  k_staged_phase<TYPE, CW><<<grid, ST_THREADS, C::SMEM_BYTES, c->stream>>>(a);
+  return IC_OK;
+}
+static bool staged_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L >= 4 * ST_SEG; }
+static bool tiled_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L <= 4 * ST_SEG; }   // one tile per row quad
+static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
+  const long long ntasks = ((long long)(c->L / 4) * (c->L / 4 / ST_SEG)) / 2;
+  const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
+  dim3 grid((unsigned)std::min(ntasks, cap), (unsigned)c->replicas);
+  a.desc16 = c->d_desc16;
+  int rc;
+  if (a.type == 0) {
+    switch (((a.p1 >> 2) & 15) >> 2) {
+      case 0: rc = launch_staged_one<PH_FAR, 0>(c, a, grid); break;
+      case 1: rc = launch_staged_one<PH_FAR, 1>(c, a, grid); break;
+      case 2: rc = launch_staged_one<PH_FAR, 2>(c, a, grid); break;
+      default: rc = launch_staged_one<PH_FAR, 3>(c, a, grid); break;
+    }
+  } else if (a.p1 == 0) rc = launch_staged_one<PH_NEAR_H, 0>(c, a, grid);
+  else rc = launch_staged_one<PH_NEAR_V, 0>(c, a, grid);
+  if (rc != IC_OK) return rc;
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
 static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_trace) {
   if (!c || !h_T) return IC_ERR_NULL;
   if (nsweeps < 0 || c->sweep + (uint64_t)nsweeps >= (1ull << 31)) return IC_ERR_PARAM;
@@ -399,7 +463,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
   }
 
   PhaseArgs a;
-  a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.desc16 = c->d_desc16; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
   a.L = c->L; a.logL = c->logL; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const double qJ = 0.25 * c->J;
   for (int64_t s = 0; s < nsweeps; ++s) {
@@ -408,8 +472,9 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     a.type = par[0]; a.p1 = par[1]; a.p2 = par[2];
     for (int phase = 0; phase < 2; ++phase) {
       a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
-      const bool tiled = c->layout == LAY_P16 && c->variant != 1;
-      int rc = tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
+      const bool staged = staged_ok(c) && (c->variant == 3 || (c->variant == 0 && c->L > 4 * ST_SEG));
+      const bool tiled = tiled_ok(c) && (c->variant == 0 || c->variant == 2);
+      int rc = staged ? launch_phase_staged(c, a) : tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
       if (rc != IC_OK) return rc;
     }
     k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ,
@@ -500,8 +565,9 @@ extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->lau
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {
   if (!c) return IC_ERR_NULL;
-  if (variant < 0 || variant > 2) return IC_ERR_PARAM;
-  if (variant == 2 && c->layout != LAY_P16) return IC_ERR_PARAM;
+  if (variant < 0 || variant > 3) return IC_ERR_PARAM;
+  if (variant == 2 && !tiled_ok(c)) return IC_ERR_PARAM;
+  if (variant == 3 && !staged_ok(c)) return IC_ERR_PARAM;
   c->variant = variant;
   return IC_OK;
 }

@@ -51,15 +51,30 @@ IC_HD int sg_of(int c) { return (c & 2) ? 0 : 1 - 2 * (c & 1); }
 // Lattice layouts in device memory.
 //   ROW8  one byte per site, public code, row-major [y][x]                       (8 bits/site, L < 64)
 //   ROW2  2 bits per site, public code, 16 sites per 32-bit word, row-major       (2 bits/site)
-//   P16   one byte per site in 16 planes [y&3][x&3][y>>2][x>>2]; byte e = f | g<<3 with
-//         (f,g) = sigma+ (1,0), sigma- (0,1), S+ (1,1), S- (0,0), so that the byte-wise sum of the four
-//         neighbour bytes is F | G<<3 with  sum S = F+G-4,  sum sigma = F-G        (8 bits/site, L >= 64)
-// Every phase of schedule S1 updates whole planes of P16, so the tiled kernels work on dense 16-byte vectors.
+//   P16   one byte per site, tiled: the lattice is cut into tiles of 4 rows x 4*SEGL columns (SEGL = min(L/4, 512));
+//         a tile is stored contiguously as 16 "plane rows" [y&3][x&3] of SEGL bytes (plane column X = x>>2 inside the
+//         tile), tiles in the order [y>>2][X / SEGL].  Byte e = f | g<<3 with (f,g) = sigma+ (1,0), sigma- (0,1),
+//         S+ (1,1), S- (0,0), so that the byte-wise sum of the four neighbour bytes is F | G<<3 with
+//         sum S = F+G-4,  sum sigma = F-G                                          (8 bits/site, L >= 64)
+// Every phase of schedule S1 updates whole plane rows of P16, so the kernels work on dense 16-byte vectors, and a
+// tile (8 KB at SEGL = 512) plus its neighbour rows is what one bulk copy stages in shared memory.
 // ---------------------------------------------------------------------------------------------------
 enum Layout : int { LAY_ROW8 = 0, LAY_ROW2 = 1, LAY_P16 = 2 };
 
 IC_HD int e_of_code(int c) { return (~c & 1) | (((c ^ (c >> 1)) & 1) << 3); }
 IC_HD int code_of_e(int e) { int b0 = ~e & 1; return b0 | ((((e >> 3) ^ b0) & 1) << 1); }
+
+// P16 addressing: lw = log2(L/4); byte offset of plane row (ky, kx) of tile (Y, seg)
+constexpr int P16_LOGSEG_MAX = 9;
+IC_HD int p16_logseg(int lw) { return lw < P16_LOGSEG_MAX ? lw : P16_LOGSEG_MAX; }
+IC_HD long long p16_row(int lw, int ky, int kx, int Y, int seg) {
+  const int ls = p16_logseg(lw);
+  return ((((long long)Y << (lw - ls)) + seg) * 16 + (ky * 4 + kx)) << ls;
+}
+IC_HD long long p16_site(int lw, int x, int y) {
+  const int ls = p16_logseg(lw), X = x >> 2;
+  return p16_row(lw, y & 3, x & 3, y >> 2, X >> ls) + (X & ((1 << ls) - 1));
+}
 
 struct LatView {              // one replica
   char* base;
@@ -69,8 +84,7 @@ struct LatView {              // one replica
 template <int LAY>
 struct Sites {
   static __device__ __forceinline__ long long p16_offset(const LatView& v, int x, int y) {
-    const int lw = v.logL - 2;
-    return ((((long long)((y & 3) * 4 + (x & 3)) << lw) + (y >> 2)) << lw) + (x >> 2);
+    return p16_site(v.logL - 2, x, y);
   }
   static __device__ __forceinline__ int load(const LatView& v, int x, int y) {
     if (LAY == LAY_P16) return code_of_e(((const uint8_t*)v.base)[p16_offset(v, x, y)]);
@@ -109,6 +123,7 @@ struct PhaseArgs {
   void* lattice;                 // [replicas][lat_stride bytes]
   const uint2* thr;              // [replicas][THR_STRIDE] (8*t29-1, packed deltas)
   const uint2* desc;             // move descriptors of this sweep type (tiled kernels), [28*8]
+  const uint4* desc16;           // 16-byte move descriptors of both sweep types (staged kernels), [28][2][8]
   ReplicaObs* obs;               // [replicas]
   long long lat_stride;          // bytes per replica
   int L, logL;

@@ -117,15 +117,15 @@ __device__ __forceinline__ void process4(uint32_t& A4, uint32_t& B4, uint32_t EA
 
 // left+right neighbour sums of the two vectors (kx = sel, sel+2) of one lattice row, from the two other planes of the row
 __device__ __forceinline__ void xnbr_sums(const uint8_t* lat, int lw, int W, int ky, int Y, int sel, int X0, V16& s_lo, V16& s_hi) {
-  const uint8_t* r0 = lat + ((((long long)(ky * 4 + sel + 1) << lw) + Y) << lw);             // plane between lo and hi
-  const uint8_t* r1 = lat + ((((long long)(ky * 4 + ((sel + 3) & 3)) << lw) + Y) << lw);     // plane right of hi / left of lo
+  const uint8_t* r0 = lat + p16_row(lw, ky, sel + 1, Y, 0);             // plane between lo and hi
+  const uint8_t* r1 = lat + p16_row(lw, ky, (sel + 3) & 3, Y, 0);     // plane right of hi / left of lo
   const V16 q0 = ld16(r0 + X0), q1 = ld16(r1 + X0);
   if (sel == 0) { s_lo = add(q0, shift_up(q1, r1[(X0 - 1) & (W - 1)])); s_hi = add(q0, q1); }
   else { s_lo = add(q0, q1); s_hi = add(q0, shift_down(q1, r1[(X0 + 16) & (W - 1)])); }
 }
 
 __device__ __forceinline__ const uint8_t* rowptr(const uint8_t* lat, int lw, int ky, int kx, int Y) {
-  return lat + ((((long long)(ky * 4 + kx) << lw) + Y) << lw);
+  return lat + p16_row(lw, ky, kx, Y, 0);     // lw <= 9: one tile per row quad, a plane row is a whole lattice row
 }
 
 template <int TYPE, int CW>
@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(256) k_codes_to_p16(const int8_t* codes, uint8
     const uint32_t o[4] = {__byte_perm(t0, t1, 0x5410), __byte_perm(t0, t1, 0x7632), __byte_perm(t2, t3, 0x5410), __byte_perm(t2, t3, 0x7632)};
 #pragma unroll
     for (int kx = 0; kx < 4; ++kx)
-      *reinterpret_cast<uint32_t*>(lat + ((((long long)((y & 3) * 4 + kx) << lw) + (y >> 2)) << lw) + 4 * j) = o[kx];
+      *reinterpret_cast<uint32_t*>(lat + p16_site(lw, 16 * j + kx, y)) = o[kx];
   }
 }
 __global__ void __launch_bounds__(256) k_p16_to_codes(const uint8_t* lat, int8_t* codes, int logL) {
@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(256) k_p16_to_codes(const uint8_t* lat, int8_t
     uint32_t p[4];
 #pragma unroll
     for (int kx = 0; kx < 4; ++kx)
-      p[kx] = *reinterpret_cast<const uint32_t*>(lat + ((((long long)((y & 3) * 4 + kx) << lw) + (y >> 2)) << lw) + 4 * j);
+      p[kx] = *reinterpret_cast<const uint32_t*>(lat + p16_site(lw, 16 * j + kx, y));
     const uint32_t t0 = __byte_perm(p[0], p[1], 0x5140), t1 = __byte_perm(p[2], p[3], 0x5140);
     const uint32_t t2 = __byte_perm(p[0], p[1], 0x7362), t3 = __byte_perm(p[2], p[3], 0x7362);
     const uint32_t e[4] = {__byte_perm(t0, t1, 0x5410), __byte_perm(t0, t1, 0x7632), __byte_perm(t2, t3, 0x5410), __byte_perm(t2, t3, 0x7632)};

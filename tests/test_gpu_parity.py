@@ -302,17 +302,18 @@ def test_config_c5_full_size_sampled(pkg):
 
 
 # ------------------------------------------------------------------------------------------------ kernel variants
-@pytest.mark.parametrize("L,reps,nsweeps", [(64, 3, 64), (128, 2, 64), (256, 2, 48), (1024, 1, 40), (4096, 1, 12)])
-def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps):
-    """Variant 2 (tiled, 16-plane layout) against variant 1 (one thread per pair) on the same device memory layout,
-    sweep by sweep so that many (mx, my) masks, both domino orientations and all four offsets are exercised; the
-    reference kernels are themselves compared with the oracle above and (at L <= 256) here."""
+@pytest.mark.parametrize("L,reps,nsweeps,variant", [(64, 3, 64, 2), (128, 2, 64, 2), (256, 2, 48, 2), (1024, 1, 40, 2),
+                                                    (2048, 2, 32, 2), (2048, 2, 48, 3), (4096, 2, 32, 3), (8192, 1, 12, 3)])
+def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant):
+    """Variant 2 (tiled, L <= 2048) and variant 3 (TMA-staged, L >= 2048) against variant 1 (one thread per pair) on the
+    same device memory layout, sweep by sweep so that many (mx, my) masks, both domino orientations and all four offsets
+    are exercised; the reference kernels are themselves compared with the oracle above and (at L <= 256) here."""
     seed = 4242 + L
     nplus, nminus = L * L // 10, L * L // 20
     n = (nplus - nminus) / (L * L)
     Ts = [0.4, 1.1, 2.5][:reps]
     codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
-    a = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); a.set_variant(2)
+    a = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); a.set_variant(variant)
     b = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); b.set_variant(1)
     for r in range(reps):
         a.set_state(r, codes[r]); b.set_state(r, codes[r])
@@ -329,4 +330,39 @@ def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps):
     if L <= 256:
         lats, _ = oracle_run(codes, 0.3, 1.0, 1.5, seed, Ts, nsweeps)
         check_against_oracle(a, lats, Ts)
+    a.close(); b.close()
+
+
+def test_staged_kernels_against_oracle_l2048(pkg):
+    """Variant 3 (TMA-staged regions) at its smallest size against the oracle: several FAR and NEAR sweeps, 2 replicas."""
+    L, seed, nsw = 2048, 77, 6
+    nplus, nminus = L * L // 8, L * L // 16
+    Ts = [0.7, 1.9]
+    codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(2)]
+    sim = pkg.Sim(L, (nplus - nminus) / (L * L), -0.5, 1.0, 2.0, seed=seed, replicas=2); sim.set_variant(3)
+    for r in range(2):
+        sim.set_state(r, codes[r])
+    sim.sweep(Ts, nsw)
+    lats = [oracle.Lattice(codes[r], -0.5, 1.0, 2.0, seed, replica=r) for r in range(2)]
+    for r in range(2):
+        lats[r].sweep_s1(Ts[r], nsw, threads=NCPU)
+    check_against_oracle(sim, lats, Ts)
+    sim.close()
+
+
+def test_staged_kernels_self_partnered_regions(pkg):
+    """FAR sweep whose mask keeps every staged region its own partner (my < 4 and mx < 2048 at L = 2048): the seed is
+    searched with the oracle's schedule function; one FAR + one NEAR sweep against the oracle and the reference kernels."""
+    L = 2048
+    seed = next(sd for sd in range(1, 200000) if oracle.schedule_params(L, sd, 0)[2] < 4)
+    typ, mx, my, _ = oracle.schedule_params(L, seed, 0)
+    assert typ == 0 and my < 4
+    code = ic_inputs.random_state(L, L * L // 10, L * L // 10, seed)
+    a = pkg.Sim(L, 0.0, 0.5, 1.0, 1.0, seed=seed); a.set_variant(3); a.set_state(0, code)
+    b = pkg.Sim(L, 0.0, 0.5, 1.0, 1.0, seed=seed); b.set_variant(1); b.set_state(0, code)
+    assert tuple(a.schedule(0)) == (typ, mx, my, 0)
+    lat = oracle.Lattice(code, 0.5, 1.0, 1.0, seed)
+    a.sweep(1.2, 2); b.sweep(1.2, 2); lat.sweep_s1(1.2, 2, threads=NCPU)
+    assert np.array_equal(a.state(0), b.state(0))
+    check_against_oracle(a, [lat], [1.2])
     a.close(); b.close()
