@@ -28,7 +28,7 @@ struct ic_ctx {
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint2* d_thr; uint2* d_desc; uint4* d_desc16; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
   // host (pinned)
   uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
@@ -61,7 +61,7 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   b += align256(lattice_bytes(L, bits)) * (size_t)replicas;       // lattices
   b += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));    // class tables (threshold, packed deltas)
   b += align256(2 * DESC_ENTRIES * sizeof(uint2));                 // move descriptors, FAR and NEAR
-  b += align256(ST_DESC_BYTES);                                    // 16-byte move descriptors (staged kernels)
+  b += align256(2 * ST_DESC_ENTRIES * sizeof(uint2));              // move descriptors of the staged kernels
   b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
   b += 256;                                                        // scratch for ic_debug_recompute
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
@@ -138,19 +138,18 @@ static void build_descriptors(int adj, uint2* out) {
     }
 }
 
-// The same table for the staged kernels: 16-byte entries at [key][adj][r] (key*256 + adj*128 + r*16 bytes):
-//   x = the four int8 coefficients, y = 8*K (byte offset of the class base in the class table),
-//   z = xor of the site bytes | (dM & 15 | (dD & 15) << 4) << 8, w = 0.
-static void build_descriptors16(uint4* out) {
+// The same table for the staged kernels, entry [adj][key*8 + r] = (coef, info):
+//   coef = the four int8 coefficients; info = 4*K (byte offset of the class base in the 4-byte threshold table) |
+//   (xor of the site bytes: a at bits 0,3, b at bits 1,4) << 16.
+static void build_descriptors32(uint2* out) {
   std::vector<uint2> d8(DESC_ENTRIES);
   for (int adj = 0; adj < 2; ++adj) {
     build_descriptors(adj, d8.data());
-    for (int key = 0; key < 28; ++key)
-      for (int r = 0; r < 8; ++r) {
-        const uint2 d = d8[key * 8 + r];
-        uint4 q; q.x = d.x; q.y = d.y & 0x7FFFu; q.z = ((d.y >> 16) & 0xFFu) | (((d.y >> 24) & 0xFFu) << 8); q.w = 0u;
-        out[key * 16 + adj * 8 + r] = q;
-      }
+    for (int e = 0; e < ST_DESC_ENTRIES; ++e) {
+      uint2 q; q.x = 0u; q.y = 4u * (uint32_t)class_index(0, 0, 0);
+      if (e < DESC_ENTRIES) { const uint2 d = d8[e]; q.x = d.x; q.y = ((d.y & 0x7FFFu) >> 1) | (((d.y >> 16) & 0xFFu) << 16); }
+      out[adj * ST_DESC_ENTRIES + e] = q;
+    }
   }
 }
 
@@ -263,7 +262,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   c->lattice = p; c->lat_stride = (long long)align256(lattice_bytes(L, bits)); p += (size_t)c->lat_stride * replicas;
   c->d_thr = (uint2*)p; p += align256((size_t)replicas * THR_STRIDE * sizeof(uint2));
   c->d_desc = (uint2*)p; p += align256(2 * DESC_ENTRIES * sizeof(uint2));
-  c->d_desc16 = (uint4*)p; p += align256(ST_DESC_BYTES);
+  c->d_desc32 = (uint2*)p; p += align256(2 * ST_DESC_ENTRIES * sizeof(uint2));
   c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
   c->d_scratch8 = (long long*)p; p += 256;
   c->d_stage = (int8_t*)p;
@@ -282,11 +281,11 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
     e = cudaMemcpyAsync(c->d_desc, desc.data(), desc.size() * sizeof(uint2), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the move descriptors"));
-    std::vector<uint4> desc16(ST_DESC_BYTES / 16);
-    build_descriptors16(desc16.data());
-    e = cudaMemcpyAsync(c->d_desc16, desc16.data(), ST_DESC_BYTES, cudaMemcpyHostToDevice, c->stream);
+    std::vector<uint2> desc32(2 * ST_DESC_ENTRIES);
+    build_descriptors32(desc32.data());
+    e = cudaMemcpyAsync(c->d_desc32, desc32.data(), desc32.size() * sizeof(uint2), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the 16-byte move descriptors"));
+    if (e != cudaSuccess) return fail(cuda_fail(e, "upload of the staged kernels' move descriptors"));
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
       return fail(cuda_fail(cudaGetLastError(), "cudaDeviceGetAttribute(multiProcessorCount)"));
@@ -423,7 +422,7 @@ static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
   const long long ntasks = ((long long)(c->L / 4) * (c->L / 4 / ST_SEG)) / 2;
   const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
   dim3 grid((unsigned)std::min(ntasks, cap), (unsigned)c->replicas);
-  a.desc16 = c->d_desc16;
+  a.desc32 = c->d_desc32;
   int rc;
   if (a.type == 0) {
     switch (((a.p1 >> 2) & 15) >> 2) {
@@ -463,22 +462,24 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
   }
 
   PhaseArgs a;
-  a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.desc16 = c->d_desc16; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.desc32 = c->d_desc32; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
   a.L = c->L; a.logL = c->logL; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const double qJ = 0.25 * c->J;
   for (int64_t s = 0; s < nsweeps; ++s) {
     int32_t par[4];
     schedule_params(c->L, c->seed, c->sweep, par);
     a.type = par[0]; a.p1 = par[1]; a.p2 = par[2];
+    bool absolute = false;
     for (int phase = 0; phase < 2; ++phase) {
       a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
       const bool staged = staged_ok(c) && (c->variant == 3 || (c->variant == 0 && c->L > 4 * ST_SEG));
       const bool tiled = tiled_ok(c) && (c->variant == 0 || c->variant == 2);
+      absolute = staged;     // the staged kernels report M, Ms of the updated sites instead of their changes
       int rc = staged ? launch_phase_staged(c, a) : tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
       if (rc != IC_OK) return rc;
     }
     k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ,
-                                                               d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr);
+                                                               d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr, absolute ? 1 : 0);
     c->launches++;
     IC_CUDA(cudaGetLastError());
     c->sweep += 1;

@@ -114,8 +114,9 @@ struct ReplicaObs {
   long long n2, bV, bJ, M, Ms, Q;      // current exact integers (updated by the phase kernels)
   long long nmeas, pad0;
   double sumE, sumE2, sumM, sumM2, sumAbsM, sumMs, sumMs2, sumAbsMs;
+  long long Mnext, Msnext;             // staged kernels: M and Ms of the sites updated so far in the current sweep
 };
-static_assert(sizeof(ReplicaObs) == 128, "ReplicaObs layout");
+static_assert(sizeof(ReplicaObs) == 144, "ReplicaObs layout");
 
 // Parameters of one phase of one sweep (schedule S1, U4), the same for all replicas
 // (precedent: identical maps for all lattice copies).
@@ -123,7 +124,7 @@ struct PhaseArgs {
   void* lattice;                 // [replicas][lat_stride bytes]
   const uint2* thr;              // [replicas][THR_STRIDE] (8*t29-1, packed deltas)
   const uint2* desc;             // move descriptors of this sweep type (tiled kernels), [28*8]
-  const uint4* desc16;           // 16-byte move descriptors of both sweep types (staged kernels), [28][2][8]
+  const uint2* desc32;           // move descriptors (coefficients, info) of both sweep types (staged kernels), [2][256]
   ReplicaObs* obs;               // [replicas]
   long long lat_stride;          // bytes per replica
   int L, logL;

@@ -10,7 +10,8 @@
 namespace ic {
 
 // Sum of five per-thread integers over the block, then one atomicAdd per value into the replica record.
-__device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV, int dJ, int dM, int dMs) {
+// absolute = false: dM, dMs are changes of M, Ms; true: they are the M, Ms of the sites updated (added to Mnext, Msnext).
+__device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV, int dJ, int dM, int dMs, bool absolute = false) {
   __shared__ int red[5][32];
   const unsigned full = 0xFFFFFFFFu;
   dn2 = __reduce_add_sync(full, dn2); dV = __reduce_add_sync(full, dV); dJ = __reduce_add_sync(full, dJ);
@@ -26,8 +27,8 @@ __device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV,
       if (v[0]) atomicAdd((unsigned long long*)&o->n2, (unsigned long long)(long long)v[0]);
       if (v[1]) atomicAdd((unsigned long long*)&o->bV, (unsigned long long)(long long)v[1]);
       if (v[2]) atomicAdd((unsigned long long*)&o->bJ, (unsigned long long)(long long)v[2]);
-      if (v[3]) atomicAdd((unsigned long long*)&o->M, (unsigned long long)(long long)v[3]);
-      if (v[4]) atomicAdd((unsigned long long*)&o->Ms, (unsigned long long)(long long)v[4]);
+      if (v[3]) atomicAdd((unsigned long long*)(absolute ? &o->Mnext : &o->M), (unsigned long long)(long long)v[3]);
+      if (v[4]) atomicAdd((unsigned long long*)(absolute ? &o->Msnext : &o->Ms), (unsigned long long)(long long)v[4]);
     }
   }
 }
@@ -114,10 +115,11 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
 
 // U5: after a sweep, E = Delta*n2 + V*bV + (J/4)*bJ and the running sums, one thread per
 // replica, IEEE fp64 with one rounding per operation (no FMA contraction: explicit _rn intrinsics).
-__global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row) {
+__global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row, int absolute) {
   int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= replicas) return;
   ReplicaObs* o = &obs[r];
+  if (absolute) { o->M = o->Mnext; o->Ms = o->Msnext; o->Mnext = 0; o->Msnext = 0; }   // the two phases covered every site once
   const double E = __dadd_rn(__dadd_rn(__dmul_rn(delta, (double)o->n2), __dmul_rn(V, (double)o->bV)),
                              __dmul_rn(quarterJ, (double)o->bJ));
   const double M = (double)o->M, Ms = (double)o->Ms;

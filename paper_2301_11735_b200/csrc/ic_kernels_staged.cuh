@@ -28,7 +28,7 @@ constexpr int ST_NPROD = 4;                   // producer warps per block
 constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane columns per region = per tile of the layout
 constexpr int ST_TPG = ST_SEG / 4;            // consumer threads per group: one 32-pair item each per task
 constexpr int ST_THREADS = 32 * ST_NPROD + ST_GROUPS * ST_TPG;
-constexpr int ST_DESC_BYTES = 28 * 256;       // 16-byte move descriptors: key*256 + adj*128 + r*16
+constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) as two 4-byte tables: coefficients, info
 
 template <int TYPE>
 struct StagedCfg {
@@ -40,9 +40,9 @@ struct StagedCfg {
   static constexpr int NSTAGE = TYPE == PH_NEAR_V ? 6 : 7;
   static constexpr int TASK_TX = 2 * (16 + 4 + (ROWS - 20)) * ST_SEG;   // bytes the bulk copies of one task deliver
   // dynamic shared memory map (byte offsets)
-  static constexpr int OFF_THR = 0;                                 // uint2[THR_STRIDE]
-  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint4 descriptors, both sweep types
-  static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_BYTES;        // NSTAGE stage buffers
+  static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
+  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint32 coef[256], then uint32 info[256]
+  static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_ENTRIES * 8;  // NSTAGE stage buffers
   static constexpr int OFF_BAR = OFF_STAGE + NSTAGE * STAGE_BYTES;  // full[NSTAGE], empty[NSTAGE]
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGE * 8 + 16;
 };
@@ -124,39 +124,56 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Four coupled pairs (one 32-bit word of site bytes per side), 16-byte move descriptors:
-//   d.x = int8 x 4 coefficients, d.y = byte offset of the class base in the class table,
-//   d.z = byte 0: xor of the site bytes (a at bits 0,3; b at bits 1,4), byte 1: dM & 15 | (dD & 15) << 4.
+// Four coupled pairs (one 32-bit word of site bytes per side).  All table lookups are 4-byte shared loads: the phase
+// kernels are bound by shared-memory wavefronts, and with 4-byte entries the hot entries of each table (sigma-sigma pairs,
+// classes without charged neighbours) fall into distinct banks.
+//   move descriptor [key*8 + r], key = fa | fb<<1 | ga<<3 | gb<<4, r = w & 7 (the table of two-site configurations,
+//   PAPER.md:66-74):  coef = four int8 coefficients;  info = byte offset of the class base in the threshold table (low 16
+//   bits) | xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
+//   class tables [class]: threshold 8*t29 - 1 (accept iff w <= it), packed (dn2, dV, dJ).
 // ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t lds_tab32(uint32_t addr) {
+  uint32_t v;
+  asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ void pairs4(uint32_t& A4, uint32_t& B4, uint32_t EA4, uint32_t EB4, uint32_t w0, uint32_t w1,
-                                       uint32_t w2, uint32_t w3, uint32_t s_desc, uint32_t s_thr, ItemAcc& acc) {
-  const uint32_t FA = (EA4 << 3) & 0x38383838u, GA = EA4 & 0x38383838u;
-  const uint32_t FB = (EB4 << 3) & 0x38383838u, GB = EB4 & 0x38383838u;
+                                       uint32_t w2, uint32_t w3, uint32_t s_desc, uint32_t s_thr, int& a3) {
+  // neighbour sums scaled by 4: the dp4a below yields a byte offset into the table of 4-byte thresholds
+  const uint32_t FA = (EA4 << 2) & 0x1C1C1C1Cu, GA = (EA4 >> 1) & 0x1C1C1C1Cu;
+  const uint32_t FB = (EB4 << 2) & 0x1C1C1C1Cu, GB = (EB4 >> 1) & 0x1C1C1C1Cu;
   const uint32_t t0 = __byte_perm(FA, GA, 0x5140), t1 = __byte_perm(FA, GA, 0x7362);
   const uint32_t u0 = __byte_perm(FB, GB, 0x5140), u1 = __byte_perm(FB, GB, 0x7362);
   const uint32_t W0 = __byte_perm(t0, u0, 0x5410), W1 = __byte_perm(t0, u0, 0x7632);
   const uint32_t W2 = __byte_perm(t1, u1, 0x5410), W3 = __byte_perm(t1, u1, 0x7632);
-  const uint32_t KEY = A4 + 2u * B4;                      // per byte: fa | fb<<1 | ga<<3 | gb<<4  (< 28)
-  // descriptor address: key * 256 (byte i of KEY moved to byte 1) + (w & 7) * 16
-  const uint4 d0 = lds_tab128(s_desc + __byte_perm(KEY, 0u, 0x4404) + ((w0 & 7u) << 4));
-  const uint4 d1 = lds_tab128(s_desc + __byte_perm(KEY, 0u, 0x4414) + ((w1 & 7u) << 4));
-  const uint4 d2 = lds_tab128(s_desc + __byte_perm(KEY, 0u, 0x4424) + ((w2 & 7u) << 4));
-  const uint4 d3 = lds_tab128(s_desc + __byte_perm(KEY, 0u, 0x4434) + ((w3 & 7u) << 4));
-  const uint2 c0 = lds_tab64(s_thr + (uint32_t)__dp4a((int)W0, (int)d0.x, (int)d0.y));
-  const uint2 c1 = lds_tab64(s_thr + (uint32_t)__dp4a((int)W1, (int)d1.x, (int)d1.y));
-  const uint2 c2 = lds_tab64(s_thr + (uint32_t)__dp4a((int)W2, (int)d2.x, (int)d2.y));
-  const uint2 c3 = lds_tab64(s_thr + (uint32_t)__dp4a((int)W3, (int)d3.x, (int)d3.y));
-  uint32_t D4 = 0u, MD4 = 0u;
-  if (w0 <= c0.x) { acc.a3 += (int)c0.y; D4 = __byte_perm(D4, d0.z, 0x3214); MD4 = __byte_perm(MD4, d0.z, 0x3215); }
-  if (w1 <= c1.x) { acc.a3 += (int)c1.y; D4 = __byte_perm(D4, d1.z, 0x3240); MD4 = __byte_perm(MD4, d1.z, 0x3250); }
-  if (w2 <= c2.x) { acc.a3 += (int)c2.y; D4 = __byte_perm(D4, d2.z, 0x3410); MD4 = __byte_perm(MD4, d2.z, 0x3510); }
-  if (w3 <= c3.x) { acc.a3 += (int)c3.y; D4 = __byte_perm(D4, d3.z, 0x4210); MD4 = __byte_perm(MD4, d3.z, 0x5210); }
+  const uint32_t KEY8 = (A4 + 2u * B4) << 3;              // per byte: 8 * key  (key < 28)
+  const uint32_t e0 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4440) | (w0 & 7u));
+  const uint32_t e1 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4441) | (w1 & 7u));
+  const uint32_t e2 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4442) | (w2 & 7u));
+  const uint32_t e3 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4443) | (w3 & 7u));
+  const uint32_t f0 = lds_tab32(e0), i0 = lds_tab32(e0 + 4u * ST_DESC_ENTRIES);
+  const uint32_t f1 = lds_tab32(e1), i1 = lds_tab32(e1 + 4u * ST_DESC_ENTRIES);
+  const uint32_t f2 = lds_tab32(e2), i2 = lds_tab32(e2 + 4u * ST_DESC_ENTRIES);
+  const uint32_t f3 = lds_tab32(e3), i3 = lds_tab32(e3 + 4u * ST_DESC_ENTRIES);
+  const uint32_t o0 = s_thr + (uint32_t)__dp4a((int)W0, (int)f0, (int)(i0 & 0xFFFFu));
+  const uint32_t o1 = s_thr + (uint32_t)__dp4a((int)W1, (int)f1, (int)(i1 & 0xFFFFu));
+  const uint32_t o2 = s_thr + (uint32_t)__dp4a((int)W2, (int)f2, (int)(i2 & 0xFFFFu));
+  const uint32_t o3 = s_thr + (uint32_t)__dp4a((int)W3, (int)f3, (int)(i3 & 0xFFFFu));
+  const uint32_t c0 = lds_tab32(o0), c1 = lds_tab32(o1), c2 = lds_tab32(o2), c3 = lds_tab32(o3);
+  uint32_t D4 = 0u;
+  if (w0 <= c0) { a3 += (int)lds_tab32(o0 + 4u * THR_STRIDE); D4 = __byte_perm(D4, i0, 0x3216); }
+  if (w1 <= c1) { a3 += (int)lds_tab32(o1 + 4u * THR_STRIDE); D4 = __byte_perm(D4, i1, 0x3260); }
+  if (w2 <= c2) { a3 += (int)lds_tab32(o2 + 4u * THR_STRIDE); D4 = __byte_perm(D4, i2, 0x3610); }
+  if (w3 <= c3) { a3 += (int)lds_tab32(o3 + 4u * THR_STRIDE); D4 = __byte_perm(D4, i3, 0x6210); }
   A4 ^= D4 & 0x09090909u;
   B4 ^= (D4 >> 1) & 0x09090909u;
-  acc.m16 = __dp4a((int)((MD4 << 4) & 0xF0F0F0F0u), 0x01010101, acc.m16);   // 16 * sum (dsig_a + dsig_b)
-  acc.d16 = __dp4a((int)(MD4 & 0xF0F0F0F0u), 0x01010101, acc.d16);          // 16 * sum (dsig_a - dsig_b)
 }
-
+// sum over the 16 site bytes f | g<<3 of a vector: accF += sum f, accT += sum f + 8 sum g
+__device__ __forceinline__ void sigma_sums(const V16& v, int& accF, int& accT) {
+  const uint32_t s = v.w[0] + v.w[1] + v.w[2] + v.w[3];     // per byte: (sum f) | (sum g) << 3, both <= 4
+  accT = __dp4a((int)s, 0x01010101, accT);
+  accF = __dp4a((int)(s & 0x07070707u), 0x01010101, accF);
+}
 
 // neighbour sums in x of the two vectors (planes sel, sel+2) of one lattice row; r0 = the 16 bytes of the plane between
 // them, r1 = of the plane on the other side, e = the byte of r1 just left (sel = 0) / right (sel = 1) of them
@@ -187,11 +204,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
   const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
   const uint32_t bar0 = smem_u32(smem + C::OFF_BAR);                    // full[s] at bar0 + 8 s, empty[s] at + 8 (NST + s)
   {
-    const uint4* src = reinterpret_cast<const uint4*>(A.thr + (long long)r * THR_STRIDE);
-    uint4* dst = reinterpret_cast<uint4*>(smem + C::OFF_THR);
-    for (int k = tid; k < THR_STRIDE / 2; k += ST_THREADS) dst[k] = __ldg(&src[k]);
-    uint4* ddst = reinterpret_cast<uint4*>(smem + C::OFF_DESC);
-    for (int k = tid; k < ST_DESC_BYTES / 16; k += ST_THREADS) ddst[k] = __ldg(&A.desc16[k]);
+    const uint2* src = A.thr + (long long)r * THR_STRIDE;
+    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
+    for (int k = tid; k < THR_STRIDE; k += ST_THREADS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+    const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
+    uint32_t* desc_s = reinterpret_cast<uint32_t*>(smem + C::OFF_DESC);
+    for (int k = tid; k < ST_DESC_ENTRIES; k += ST_THREADS) { const uint2 v = __ldg(&dsrc[k]); desc_s[k] = v.x; desc_s[ST_DESC_ENTRIES + k] = v.y; }
     if (tid == 0) {
       for (int s = 0; s < NST; ++s) {
         mbar_init(bar0 + 8 * s, 2);                                     // producer lane 0: expect_tx, and after the edge bytes
@@ -218,6 +236,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
   };
   // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n uses ring slot n % NST
   int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
+  int aF = 0, aT = 0, bF = 0, bT = 0, sgn = 1;   // sums over the new site bytes of the a- and b-sites (sigma_sums)
 
   if (tid < 32 * ST_NPROD) {
     // ============================== producer warps: warp p fills the ring slots s with s % ST_NPROD == p ================
@@ -283,7 +302,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     const int ct = tid - 32 * ST_NPROD, g = ct / ST_TPG, tg = ct - g * ST_TPG;
     const int sub = tg >> 5, chunk = tg & 31, U = sub >> 1, half = sub & 1, X0 = chunk << 4;   // SEG / 16 = 32 chunks
     const uint32_t s_thr = smem_u32(smem + C::OFF_THR);
-    const uint32_t s_desc = smem_u32(smem + C::OFF_DESC) + (TYPE == PH_FAR ? 0u : 128u);
+    const uint32_t s_desc = smem_u32(smem + C::OFF_DESC);
     const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
     // byte offsets inside a stage buffer: the 16 bytes at plane column Xc of staged row (ky_rel, kx) of region UU,
     // and the bytes just left / right of them (across the tile edge: the side array filled by the producer)
@@ -302,8 +321,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
       const int Y = mp->Y, chunkG = (mp->S0 >> 4) + chunk;
       uint8_t* const gpa = reinterpret_cast<uint8_t*>(mp->pa);
       uint8_t* const gpb = reinterpret_cast<uint8_t*>(mp->pb);
-      ItemAcc acc; acc.a3 = 0; acc.m16 = 0; acc.d16 = 0;
-      int sgn;
+      int a3 = 0;
 
       if (TYPE == PH_FAR || TYPE == PH_NEAR_V) {
         int sel, ky, kyb_r, UB, kxb_lo, kxb_hi, Xb = X0;
@@ -360,10 +378,11 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
         for (int j = 0; j < 4; ++j) {
           const u32x4 r0 = philox4x32_10((uint32_t)(8 * chunkG + 2 * j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
           const u32x4 r1 = philox4x32_10((uint32_t)(8 * chunkG + 2 * j + 1), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-          pairs4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[2], r1.v[0], r1.v[2], s_desc, s_thr, acc);
-          pairs4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r0.v[1], r0.v[3], r1.v[1], r1.v[3], s_desc, s_thr, acc);
+          pairs4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[2], r1.v[0], r1.v[2], s_desc, s_thr, a3);
+          pairs4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r0.v[1], r0.v[3], r1.v[1], r1.v[3], s_desc, s_thr, a3);
         }
         if (TYPE == PH_FAR) { b_lo = xor_perm<CW>(b_lo, selb); b_hi = xor_perm<CW>(b_hi, selb); }
+        sigma_sums(a_lo, aF, aT); sigma_sums(a_hi, aF, aT); sigma_sums(b_lo, bF, bT); sigma_sums(b_hi, bF, bT);
         st16(gpa + X0, a_lo); st16(gpa + 2 * SEG + X0, a_hi);
         st16(gpb + Xb, b_lo); st16(gpb + (kxb_hi - kxb_lo) * SEG + Xb, b_hi);
       } else {
@@ -387,8 +406,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
             const u32x4 rr = philox4x32_10((uint32_t)(4 * chunkG + j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-            pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, s_thr, acc);
+            pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, s_thr, a3);
           }
+          sigma_sums(a, aF, aT); sigma_sums(b, bF, bT);
           st16(gpb + 8 * v * SEG + X0, b);                                       // plane row (ky, kb): 8 rows below for v = 1
           if (sh_a == 0) st16(gpa + 8 * v * SEG + X0, a);
           else st16_left1_tile(gpa + 8 * v * SEG, reinterpret_cast<uint8_t*>(mp->pl) + 8 * v * SEG, X0, a);
@@ -397,15 +417,17 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
       __syncwarp();
       if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
       // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
-      int tt = acc.a3;
-      const int j11 = (tt << 21) >> 21; tt = (tt - j11) >> 11;
-      const int v11 = (tt << 21) >> 21; tt = (tt - v11) >> 11;
-      tJ += j11; tV += v11; tn2 += tt;
-      tM += acc.m16 >> 4;
-      tMs += sgn * ((TYPE == PH_FAR ? acc.m16 : acc.d16) >> 4);
+      const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
+      const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
+      tJ += j11; tV += v11; tn2 += a3;
     }
+    // M and Ms of the sites this thread updated, from their new values: sum sigma = sum f - sum g = (9 accF - accT) / 8.
+    // Every site is active in exactly one phase of a sweep, so the two phases add up to the whole lattice (k_fold).
+    const int Ma = (9 * aF - aT) >> 3, Mb = (9 * bF - bT) >> 3;
+    tM = Ma + Mb;
+    tMs = sgn * (TYPE == PH_FAR ? Ma + Mb : Ma - Mb);      // FAR: all active sites have one colour; NEAR: a and b differ
   }
-  block_accumulate(&A.obs[r], tn2, tV, tJ, tM, tMs);
+  block_accumulate(&A.obs[r], tn2, tV, tJ, tM, tMs, true);
 }
 
 }  // namespace ic
