@@ -331,6 +331,14 @@ void orc_schedule_params(int L, uint64_t seed, uint64_t sweep, int32_t out4[4]) 
   }
 }
 
+/* Random-number address of the pair whose slot site is (x, y) (the a-site; the b-site for horizontal dominoes):
+ * Philox block counter c0 = 4*(X >> 2) + (x & 3) with X = x >> 2, c1 = y, and the word X & 3 of the block, so that
+ * four consecutive sites x, x+4, x+8, x+12 of one row share a block (U3).                                */
+static void rng_address(int x, int y, uint32_t* c0, uint32_t* c1, uint32_t* word) {
+  int X = x >> 2;
+  *c0 = (uint32_t)(((X >> 2) << 2) | (x & 3)); *c1 = (uint32_t)y; *word = (uint32_t)(X & 3);
+}
+
 /* The k-th candidate a-site of phase `phase` of sweep-type `par`: returns 1 and
  * fills the pair and its random-number address (c0, c1, word) if (x, y) is an
  * a-site.  Pairs of a phase are enumerated by ascending y, then ascending x.   */
@@ -340,23 +348,20 @@ static int s1_pair_at(int L, const int32_t par[4], int phase, int x, int y,
     int mx = par[1], my = par[2];
     if (((x + y) & 1) != phase || (x & 1)) return 0;
     *xb = x ^ mx; *yb = y ^ my;
-    int rank = x >> 1;
-    *c0 = (uint32_t)(rank >> 2); *c1 = (uint32_t)y; *word = (uint32_t)(rank & 3);
+    rng_address(x, y, c0, c1, word);
     return 1;
   }
   int o = par[1], off = par[2];
   if (o == 0) { /* horizontal dominoes: u = x, v = y */
     if (((x - off - 2 * ((y + phase) & 1)) & 3) != 0) return 0;
     *xb = (x + 1) % L; *yb = y;
-    int rank = *xb >> 2; /* rank by the 4-site word that holds the b-site */
-    *c0 = (uint32_t)(rank >> 2); *c1 = (uint32_t)y; *word = (uint32_t)(rank & 3);
+    rng_address(*xb, y, c0, c1, word); /* addressed by the b-site */
     return 1;
   }
   /* vertical dominoes: u = y, v = x */
   if (((y - off - 2 * ((x + phase) & 1)) & 3) != 0) return 0;
   *xb = x; *yb = (y + 1) % L;
-  int rank = x >> 1;
-  *c0 = (uint32_t)(rank >> 2); *c1 = (uint32_t)y; *word = (uint32_t)(rank & 3);
+  rng_address(x, y, c0, c1, word);
   return 1;
 }
 

@@ -139,7 +139,7 @@ static void build_descriptors(int adj, uint2* out) {
 }
 
 // The same table for the staged kernels, entry [adj][key*8 + r] = (coef, info):
-//   coef = the four int8 coefficients; info = 4*K (byte offset of the class base in the 4-byte threshold table) |
+//   coef = the four int8 coefficients (cFa, cGa/2, cFb, cGb/2); info = 4*K (byte offset of the class base in the 4-byte threshold table) |
 //   (xor of the site bytes: a at bits 0,3, b at bits 1,4) << 16.
 static void build_descriptors32(uint2* out) {
   std::vector<uint2> d8(DESC_ENTRIES);
@@ -147,7 +147,13 @@ static void build_descriptors32(uint2* out) {
     build_descriptors(adj, d8.data());
     for (int e = 0; e < ST_DESC_ENTRIES; ++e) {
       uint2 q; q.x = 0u; q.y = 4u * (uint32_t)class_index(0, 0, 0);
-      if (e < DESC_ENTRIES) { const uint2 d = d8[e]; q.x = d.x; q.y = ((d.y & 0x7FFFu) >> 1) | (((d.y >> 16) & 0xFFu) << 16); }
+      if (e < DESC_ENTRIES) {
+        const uint2 d = d8[e];
+        // the kernel feeds (4F, 8G) per site: halve the G coefficients (33 dS - dsig is even)
+        const int cFa = (int8_t)(d.x & 0xFF), cGa = (int8_t)((d.x >> 8) & 0xFF), cFb = (int8_t)((d.x >> 16) & 0xFF), cGb = (int8_t)((d.x >> 24) & 0xFF);
+        q.x = (uint32_t)(cFa & 0xFF) | ((uint32_t)((cGa / 2) & 0xFF) << 8) | ((uint32_t)(cFb & 0xFF) << 16) | ((uint32_t)((cGb / 2) & 0xFF) << 24);
+        q.y = ((d.y & 0x7FFFu) >> 1) | (((d.y >> 16) & 0xFFu) << 16);
+      }
       out[adj * ST_DESC_ENTRIES + e] = q;
     }
   }

@@ -218,13 +218,13 @@ __global__ void __launch_bounds__(P16_THREADS) k_p16_phase(PhaseArgs A) {
         ea_lo = add(ea_lo, b_lo); ea_hi = add(ea_hi, b_hi);
         eb_lo = add(eb_lo, a_lo); eb_hi = add(eb_hi, a_hi);
       }
-      // random words: block (c0 = x>>3, c1 = y), word (x>>1)&3  (U3)
+      // random words: block c0 = 4*(X>>2) + kx, c1 = y, word X & 3 with X = x>>2, kx = x&3  (U3)
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        const u32x4 r0 = philox4x32_10((uint32_t)(8 * chunk + 2 * j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-        const u32x4 r1 = philox4x32_10((uint32_t)(8 * chunk + 2 * j + 1), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-        process4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[2], r1.v[0], r1.v[2], s_desc, s_thr, acc);
-        process4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r0.v[1], r0.v[3], r1.v[1], r1.v[3], s_desc, s_thr, acc);
+        const u32x4 r0 = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + sel), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        const u32x4 r1 = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + sel + 2), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        process4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[1], r0.v[2], r0.v[3], s_desc, s_thr, acc);
+        process4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r1.v[0], r1.v[1], r1.v[2], r1.v[3], s_desc, s_thr, acc);
       }
       if (TYPE == PH_FAR) { b_lo = xor_perm<CW>(b_lo, selb); b_hi = xor_perm<CW>(b_hi, selb); }
       st16(pa_lo, a_lo); st16(pa_hi, a_hi); st16(pb_lo, b_lo); st16(pb_hi, b_hi);
@@ -244,10 +244,10 @@ __global__ void __launch_bounds__(P16_THREADS) k_p16_phase(PhaseArgs A) {
                      add(ldrow(rowptr(lat, lw, kyu, ka, Yu), X0, W, sh_a), ldrow(rowptr(lat, lw, kyd, ka, Yd), X0, W, sh_a)));
         V16 eb = add(add(a, ldrow(rowptr(lat, lw, ky, (kb + 1) & 3, Y), X0, W, sh_r)),
                      add(ld16(rowptr(lat, lw, kyu, kb, Yu) + X0), ld16(rowptr(lat, lw, kyd, kb, Yd) + X0)));
-        // random words: block (c0 = xb>>4, c1 = y), word (xb>>2)&3
+        // random words, addressed by the b-site: block c0 = 4*(Xb>>2) + kb, c1 = y, word Xb & 3
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          const u32x4 rr = philox4x32_10((uint32_t)(4 * chunk + j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+          const u32x4 rr = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + kb), (uint32_t)y, A.c2, c3, A.key0, A.key1);
           process4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, s_thr, acc);
         }
         st16(pb, b);

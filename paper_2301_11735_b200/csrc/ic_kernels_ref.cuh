@@ -47,15 +47,15 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
     if (A.type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
       int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
       xa = 2 * i; ya = 2 * j + A.phase; xb = xa ^ A.p1; yb = ya ^ A.p2; adj = 0;
-      c0 = (uint32_t)xa >> 3; word = ((uint32_t)xa >> 1) & 3u;
+      c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
     } else if (A.p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
       int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
       xa = ((A.p2 + 2 * ((ya + A.phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
-      uint32_t rank = (uint32_t)xb >> 2; c0 = rank >> 2; word = rank & 3u;
+      c0 = (((uint32_t)xb >> 4) << 2) | ((uint32_t)xb & 3u); word = ((uint32_t)xb >> 2) & 3u;   // addressed by the b-site
     } else {                           // NEAR, vertical dominoes
       xa = (int)(t & mask); int jy = (int)(t >> logL);
       ya = ((A.p2 + 2 * ((xa + A.phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
-      uint32_t rank = (uint32_t)xa >> 1; c0 = rank >> 2; word = rank & 3u;
+      c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
     }
     u32x4 rnd = philox4x32_10(c0, (uint32_t)ya, A.c2, (uint32_t)r | (TAG_UPDATE << 28), A.key0, A.key1);
     uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];

@@ -23,12 +23,13 @@
 
 namespace ic {
 
-constexpr int ST_GROUPS = 4;                  // consumer groups per block
+constexpr int ST_GROUPS = 3;                  // consumer groups per block
 constexpr int ST_NPROD = 4;                   // producer warps per block
 constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane columns per region = per tile of the layout
-constexpr int ST_TPG = ST_SEG / 4;            // consumer threads per group: one 32-pair item each per task
+constexpr int ST_TPG = ST_SEG / 2;            // consumer threads per group: one 16-pair item each per task
 constexpr int ST_THREADS = 32 * ST_NPROD + ST_GROUPS * ST_TPG;
-constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) as two 4-byte tables: coefficients, info
+constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) in global memory: (coefficients, info)
+constexpr int ST_DESC_SMEM = 16 * 8 * 128;    // in shared memory: [compact key][r][lane & 15] x 8 bytes, a private copy per lane
 
 template <int TYPE>
 struct StagedCfg {
@@ -41,8 +42,8 @@ struct StagedCfg {
   static constexpr int TASK_TX = 2 * (16 + 4 + (ROWS - 20)) * ST_SEG;   // bytes the bulk copies of one task deliver
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
-  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint32 coef[256], then uint32 info[256]
-  static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_ENTRIES * 8;  // NSTAGE stage buffers
+  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [16][8][16]
+  static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_SMEM;         // NSTAGE stage buffers
   static constexpr int OFF_BAR = OFF_STAGE + NSTAGE * STAGE_BYTES;  // full[NSTAGE], empty[NSTAGE]
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGE * 8 + 16;
 };
@@ -80,6 +81,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok)
         : "r"(bar), "r"(parity)
         : "memory");
+  }
+}
+// producers are far ahead of the consumers most of the time: sleep between polls instead of burning issue slots
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  while (true) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) break;
+    __nanosleep(1000);
   }
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -127,9 +143,10 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
 // Four coupled pairs (one 32-bit word of site bytes per side).  All table lookups are 4-byte shared loads: the phase
 // kernels are bound by shared-memory wavefronts, and with 4-byte entries the hot entries of each table (sigma-sigma pairs,
 // classes without charged neighbours) fall into distinct banks.
-//   move descriptor [key*8 + r], key = fa | fb<<1 | ga<<3 | gb<<4, r = w & 7 (the table of two-site configurations,
-//   PAPER.md:66-74):  coef = four int8 coefficients;  info = byte offset of the class base in the threshold table (low 16
-//   bits) | xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
+//   move descriptor [key][r], key = fa | fb<<1 | ga<<2 | gb<<3, r = w & 7 (the table of two-site configurations,
+//   PAPER.md:66-74), 8 bytes, 16 copies so that every lane of a half warp reads its own banks (no conflicts at all):
+//   coef = four int8 coefficients;  info = shared-memory address of the class base in the threshold table (low 16 bits) |
+//   xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
 //   class tables [class]: threshold 8*t29 - 1 (accept iff w <= it), packed (dn2, dV, dJ).
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lds_tab32(uint32_t addr) {
@@ -138,27 +155,26 @@ __device__ __forceinline__ uint32_t lds_tab32(uint32_t addr) {
   return v;
 }
 __device__ __forceinline__ void pairs4(uint32_t& A4, uint32_t& B4, uint32_t EA4, uint32_t EB4, uint32_t w0, uint32_t w1,
-                                       uint32_t w2, uint32_t w3, uint32_t s_desc, uint32_t s_thr, int& a3) {
-  // neighbour sums scaled by 4: the dp4a below yields a byte offset into the table of 4-byte thresholds
-  const uint32_t FA = (EA4 << 2) & 0x1C1C1C1Cu, GA = (EA4 >> 1) & 0x1C1C1C1Cu;
-  const uint32_t FB = (EB4 << 2) & 0x1C1C1C1Cu, GB = (EB4 >> 1) & 0x1C1C1C1Cu;
+                                       uint32_t w2, uint32_t w3, uint32_t s_desc, int& a3) {
+  // neighbour sums as (4F, 8G), G coefficients halved: the dp4a below yields a byte address in the 4-byte thresholds
+  const uint32_t FA = (EA4 << 2) & 0x1C1C1C1Cu, GA = EA4 & 0x38383838u;
+  const uint32_t FB = (EB4 << 2) & 0x1C1C1C1Cu, GB = EB4 & 0x38383838u;
   const uint32_t t0 = __byte_perm(FA, GA, 0x5140), t1 = __byte_perm(FA, GA, 0x7362);
   const uint32_t u0 = __byte_perm(FB, GB, 0x5140), u1 = __byte_perm(FB, GB, 0x7362);
   const uint32_t W0 = __byte_perm(t0, u0, 0x5410), W1 = __byte_perm(t0, u0, 0x7632);
   const uint32_t W2 = __byte_perm(t1, u1, 0x5410), W3 = __byte_perm(t1, u1, 0x7632);
-  const uint32_t KEY8 = (A4 + 2u * B4) << 3;              // per byte: 8 * key  (key < 28)
-  const uint32_t e0 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4440) | (w0 & 7u));
-  const uint32_t e1 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4441) | (w1 & 7u));
-  const uint32_t e2 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4442) | (w2 & 7u));
-  const uint32_t e3 = s_desc + 4u * (__byte_perm(KEY8, 0u, 0x4443) | (w3 & 7u));
-  const uint32_t f0 = lds_tab32(e0), i0 = lds_tab32(e0 + 4u * ST_DESC_ENTRIES);
-  const uint32_t f1 = lds_tab32(e1), i1 = lds_tab32(e1 + 4u * ST_DESC_ENTRIES);
-  const uint32_t f2 = lds_tab32(e2), i2 = lds_tab32(e2 + 4u * ST_DESC_ENTRIES);
-  const uint32_t f3 = lds_tab32(e3), i3 = lds_tab32(e3 + 4u * ST_DESC_ENTRIES);
-  const uint32_t o0 = s_thr + (uint32_t)__dp4a((int)W0, (int)f0, (int)(i0 & 0xFFFFu));
-  const uint32_t o1 = s_thr + (uint32_t)__dp4a((int)W1, (int)f1, (int)(i1 & 0xFFFFu));
-  const uint32_t o2 = s_thr + (uint32_t)__dp4a((int)W2, (int)f2, (int)(i2 & 0xFFFFu));
-  const uint32_t o3 = s_thr + (uint32_t)__dp4a((int)W3, (int)f3, (int)(i3 & 0xFFFFu));
+  // compact key fa | fb<<1 | ga<<2 | gb<<3, times 4 in each byte; byte i moved to byte 1 is key * 1024 = its table row
+  const uint32_t X2 = (A4 + 2u * B4) << 1;                // per byte: fa<<1 | fb<<2 | ga<<4 | gb<<5
+  const uint32_t KS = (X2 & 0x30303030u) | ((X2 << 1) & 0x0C0C0C0Cu);
+  const uint2 q0 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4404) + ((w0 & 7u) << 7));   // s_desc includes (lane & 15) * 8
+  const uint2 q1 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4414) + ((w1 & 7u) << 7));
+  const uint2 q2 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4424) + ((w2 & 7u) << 7));
+  const uint2 q3 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4434) + ((w3 & 7u) << 7));
+  const uint32_t f0 = q0.x, i0 = q0.y, f1 = q1.x, i1 = q1.y, f2 = q2.x, i2 = q2.y, f3 = q3.x, i3 = q3.y;
+  const uint32_t o0 = (uint32_t)__dp4a((int)W0, (int)f0, (int)(i0 & 0xFFFFu));
+  const uint32_t o1 = (uint32_t)__dp4a((int)W1, (int)f1, (int)(i1 & 0xFFFFu));
+  const uint32_t o2 = (uint32_t)__dp4a((int)W2, (int)f2, (int)(i2 & 0xFFFFu));
+  const uint32_t o3 = (uint32_t)__dp4a((int)W3, (int)f3, (int)(i3 & 0xFFFFu));
   const uint32_t c0 = lds_tab32(o0), c1 = lds_tab32(o1), c2 = lds_tab32(o2), c3 = lds_tab32(o3);
   uint32_t D4 = 0u;
   if (w0 <= c0) { a3 += (int)lds_tab32(o0 + 4u * THR_STRIDE); D4 = __byte_perm(D4, i0, 0x3216); }
@@ -175,13 +191,6 @@ __device__ __forceinline__ void sigma_sums(const V16& v, int& accF, int& accT) {
   accF = __dp4a((int)(s & 0x07070707u), 0x01010101, accF);
 }
 
-// neighbour sums in x of the two vectors (planes sel, sel+2) of one lattice row; r0 = the 16 bytes of the plane between
-// them, r1 = of the plane on the other side, e = the byte of r1 just left (sel = 0) / right (sel = 1) of them
-__device__ __forceinline__ void xnbr_sums_s(const uint8_t* r0, const uint8_t* r1, const uint8_t* e, int sel, V16& s_lo, V16& s_hi) {
-  const V16 q0 = ld16(r0), q1 = ld16(r1);
-  if (sel == 0) { s_lo = add(q0, shift_up(q1, *e)); s_hi = add(q0, q1); }
-  else { s_lo = add(q0, q1); s_hi = add(q0, shift_down(q1, *e)); }
-}
 // store 16 bytes at plane columns X0-1 .. X0+14 of a tile row; the byte at -1 of the tile lives at `left`
 __device__ __forceinline__ void st16_left1_tile(uint8_t* row, uint8_t* left, int X0, const V16& v) {
   *(X0 ? row + X0 - 1 : left) = (uint8_t)(v.w[0] & 0xFFu);
@@ -208,8 +217,13 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
     for (int k = tid; k < THR_STRIDE; k += ST_THREADS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
     const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
-    uint32_t* desc_s = reinterpret_cast<uint32_t*>(smem + C::OFF_DESC);
-    for (int k = tid; k < ST_DESC_ENTRIES; k += ST_THREADS) { const uint2 v = __ldg(&dsrc[k]); desc_s[k] = v.x; desc_s[ST_DESC_ENTRIES + k] = v.y; }
+    uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
+    for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_THREADS) {
+      const int kc = k >> 7, rr = (k >> 4) & 7, key = (kc & 3) | ((kc & 12) << 1);
+      uint2 d = __ldg(&dsrc[key * 8 + rr]);
+      d.y += smem_u32(smem + C::OFF_THR);       // low 16 bits: shared-memory address of the class base (< 64 KB)
+      desc_s[k] = d;
+    }
     if (tid == 0) {
       for (int s = 0; s < NST; ++s) {
         mbar_init(bar0 + 8 * s, 2);                                     // producer lane 0: expect_tx, and after the edge bytes
@@ -244,10 +258,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, (lane >> 2) - 1, lane & 3) : 0;   // lane = staged row
     // a ring slot is always filled by the same producer warp (slot % ST_NPROD), in task order: a parity wait is only
     // safe for a waiter that is at most one phase ahead of the barrier
-    for (int n = 0, t = blockIdx.x; t < ntasks; ++n, t += gridDim.x) {
-      const int s = n % NST;
+    for (int t = blockIdx.x, s = 0, lap = 0; t < ntasks; t += gridDim.x, lap ^= (s + 1 == NST), s = (s + 1 == NST) ? 0 : s + 1) {
       if (s % ST_NPROD != p) continue;
-      mbar_wait(bar0 + 8 * (NST + s), ((n / NST) & 1) ^ 1);
+      mbar_wait_backoff(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1));
       unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       const uint32_t full = bar0 + 8 * s;
       int Yq[2], sg[2];
@@ -270,11 +283,11 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
             const int UP = paired ? (U ^ 1) : U;
             const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
             mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
-            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, mx & 3, Yq[UP], sg[UP]));
+            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yq[UP], sg[UP]));
           } else if (TYPE == PH_NEAR_V) {
             const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-            mt.pa = (unsigned long long)(lat + p16_row(lw, ky, half, Y, seg));
-            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, half, Yb, seg));
+            mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
+            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yb, seg));
           } else {
             const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
             mt.pa = (unsigned long long)(lat + p16_row(lw, half, ka, Y, seg));
@@ -300,10 +313,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
   } else {
     // =========================================== consumer warps ====================================================
     const int ct = tid - 32 * ST_NPROD, g = ct / ST_TPG, tg = ct - g * ST_TPG;
-    const int sub = tg >> 5, chunk = tg & 31, U = sub >> 1, half = sub & 1, X0 = chunk << 4;   // SEG / 16 = 32 chunks
-    const uint32_t s_thr = smem_u32(smem + C::OFF_THR);
-    const uint32_t s_desc = smem_u32(smem + C::OFF_DESC);
+    // item = one 16-byte vector of a-sites (b-sites for NEAR-H) = 16 coupled pairs: sub-task (U, half), plane/row selector
+    // hi, chunk of 16 plane columns (SEG / 16 = 32 chunks); all but the chunk are uniform in a warp
+    const int sub = tg >> 6, hi = (tg >> 5) & 1, chunk = tg & 31, U = sub >> 1, half = sub & 1, X0 = chunk << 4;
+    const uint32_t s_desc = smem_u32(smem + C::OFF_DESC) + (uint32_t)(lane & 15) * 8u;
     const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
+    auto addf = [](const V16& p, const V16& q) -> V16 { return add(p, q); };
     // byte offsets inside a stage buffer: the 16 bytes at plane column Xc of staged row (ky_rel, kx) of region UU,
     // and the bytes just left / right of them (across the tile edge: the side array filled by the producer)
     auto off = [&](int UU, int kyr, int kx, int Xc) -> int { return UU * C::REGION_BYTES + ((((kyr + 1) << 2) + (kx & 3)) << LOGSEG) + Xc; };
@@ -313,113 +328,90 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     auto offR = [&](int UU, int kyr, int kx, int Xc) -> int {
       return Xc != SEG - 16 ? off(UU, kyr, kx, Xc) + 16 : C::OFF_HALO + UU * 64 + 32 + ((kyr + 1) << 2) + (kx & 3);
     };
-    for (int n = g, t = blockIdx.x + g * gridDim.x; t < ntasks; n += ST_GROUPS, t += ST_GROUPS * gridDim.x) {
-      const int s = n % NST;
-      mbar_wait(bar0 + 8 * s, (n / NST) & 1);
+    for (int t = blockIdx.x + g * gridDim.x, s = g, lap = 0; t < ntasks; t += ST_GROUPS * gridDim.x) {
+      mbar_wait(bar0 + 8 * s, (uint32_t)lap);
       const uint8_t* st = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       const SubMeta* mp = reinterpret_cast<const SubMeta*>(st + C::OFF_SMETA) + sub;
       const int Y = mp->Y, chunkG = (mp->S0 >> 4) + chunk;
-      uint8_t* const gpa = reinterpret_cast<uint8_t*>(mp->pa);
-      uint8_t* const gpb = reinterpret_cast<uint8_t*>(mp->pb);
-      int a3 = 0;
-
-      if (TYPE == PH_FAR || TYPE == PH_NEAR_V) {
-        int sel, ky, kyb_r, UB, kxb_lo, kxb_hi, Xb = X0;
-        uint32_t selb = 0x3210u;
-        if (TYPE == PH_FAR) {
-          sel = 0; ky = A.phase + 2 * half;
-          kyb_r = ky ^ (my & 3); UB = paired ? (U ^ 1) : U;
-          kxb_lo = mx & 3; kxb_hi = 2 ^ (mx & 3);
-          Xb = X0 ^ ((mx >> 2) & (SEG - 1) & ~15);                     // the partner chunk inside the partner tile
-          const int cb = (mx >> 2) & 3;
-          selb = cb == 0 ? 0x3210u : cb == 1 ? 0x2301u : cb == 2 ? 0x1032u : 0x0123u;
-          sgn = A.phase ? -1 : 1;
-        } else {
-          sel = half; ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3;
-          kyb_r = ky + 1; UB = U;                                        // may be row 4 = row 0 of the quad below
-          kxb_lo = sel; kxb_hi = sel + 2;
-          sgn = ((sel + ky) & 1) ? -1 : 1;
-        }
-        const int y = 4 * Y + ky;
-        // a side: planes (sel, sel+2); x-neighbours are planes sel+1 and sel+3 (one byte to the left / right when wrapping)
-        V16 a_lo = ld16(st + off(U, ky, sel, X0)), a_hi = ld16(st + off(U, ky, sel + 2, X0));
-        V16 ea_lo, ea_hi;
-        xnbr_sums_s(st + off(U, ky, sel + 1, X0), st + off(U, ky, sel + 3, X0),
-                    st + (sel == 0 ? offL(U, ky, sel + 3, X0) : offR(U, ky, sel + 3, X0)), sel, ea_lo, ea_hi);
-        ea_lo = add(ea_lo, ld16(st + off(U, ky - 1, sel, X0)));
-        ea_hi = add(ea_hi, ld16(st + off(U, ky - 1, sel + 2, X0)));
-        // b side, natural lane order
-        const int selp = TYPE == PH_FAR ? 1 : sel;          // b-planes are (selp, selp + 2)
-        V16 b_lo = ld16(st + off(UB, kyb_r, kxb_lo, Xb)), b_hi = ld16(st + off(UB, kyb_r, kxb_hi, Xb));
-        V16 eb_lo, eb_hi;
-        {
-          V16 s_first, s_second;
-          xnbr_sums_s(st + off(UB, kyb_r, selp + 1, Xb), st + off(UB, kyb_r, selp + 3, Xb),
-                      st + (selp == 0 ? offL(UB, kyb_r, selp + 3, Xb) : offR(UB, kyb_r, selp + 3, Xb)), selp, s_first, s_second);
-          if (TYPE == PH_FAR) { const bool sw = (kxb_lo == 3); eb_lo = sw ? s_second : s_first; eb_hi = sw ? s_first : s_second; }
-          else { eb_lo = s_first; eb_hi = s_second; }
-          eb_lo = add(eb_lo, ld16(st + off(UB, kyb_r + 1, kxb_lo, Xb)));
-          eb_hi = add(eb_hi, ld16(st + off(UB, kyb_r + 1, kxb_hi, Xb)));
-        }
-        if (TYPE == PH_FAR) {
-          ea_lo = add(ea_lo, ld16(st + off(U, ky + 1, 0, X0)));
-          ea_hi = add(ea_hi, ld16(st + off(U, ky + 1, 2, X0)));
-          eb_lo = add(eb_lo, ld16(st + off(UB, kyb_r - 1, kxb_lo, Xb)));
-          eb_hi = add(eb_hi, ld16(st + off(UB, kyb_r - 1, kxb_hi, Xb)));
-          b_lo = xor_perm<CW>(b_lo, selb); b_hi = xor_perm<CW>(b_hi, selb);
-          eb_lo = xor_perm<CW>(eb_lo, selb); eb_hi = xor_perm<CW>(eb_hi, selb);
-        } else {
-          // vertical domino: a's lower neighbour is b, b's upper neighbour is a
-          ea_lo = add(ea_lo, b_lo); ea_hi = add(ea_hi, b_hi);
-          eb_lo = add(eb_lo, a_lo); eb_hi = add(eb_hi, a_hi);
-        }
-        // random words: block (c0 = x>>3, c1 = y), word (x>>1)&3  (U3)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const u32x4 r0 = philox4x32_10((uint32_t)(8 * chunkG + 2 * j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-          const u32x4 r1 = philox4x32_10((uint32_t)(8 * chunkG + 2 * j + 1), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-          pairs4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[2], r1.v[0], r1.v[2], s_desc, s_thr, a3);
-          pairs4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r0.v[1], r0.v[3], r1.v[1], r1.v[3], s_desc, s_thr, a3);
-        }
-        if (TYPE == PH_FAR) { b_lo = xor_perm<CW>(b_lo, selb); b_hi = xor_perm<CW>(b_hi, selb); }
-        sigma_sums(a_lo, aF, aT); sigma_sums(a_hi, aF, aT); sigma_sums(b_lo, bF, bT); sigma_sums(b_hi, bF, bT);
-        st16(gpa + X0, a_lo); st16(gpa + 2 * SEG + X0, a_hi);
-        st16(gpb + Xb, b_lo); st16(gpb + (kxb_hi - kxb_lo) * SEG + Xb, b_hi);
+      uint8_t* gpa = reinterpret_cast<uint8_t*>(mp->pa);
+      uint8_t* gpb = reinterpret_cast<uint8_t*>(mp->pb);
+      // the 16 bytes of plane kx at row kyr, shifted by one site to the left (sh < 0) or right (sh > 0) if asked
+      auto ldrow = [&](int UU, int kyr, int kx, int Xc, int sh) -> V16 {
+        V16 v = ld16(st + off(UU, kyr, kx, Xc));
+        if (sh < 0) v = shift_up(v, st[offL(UU, kyr, kx, Xc)]);
+        else if (sh > 0) v = shift_down(v, st[offR(UU, kyr, kx, Xc)]);
+        return v;
+      };
+      // left + right neighbours of the vector of plane kx: planes kx-1 and kx+1, one site over when they wrap around
+      auto xsum = [&](int UU, int kyr, int kx, int Xc) -> V16 {
+        return addf(ldrow(UU, kyr, kx + 3, Xc, kx == 0 ? -1 : 0), ldrow(UU, kyr, kx + 1, Xc, kx == 3 ? 1 : 0));
+      };
+      V16 a, b, ea, eb;
+      int y, kxr;                       // Philox counters: lattice row and plane of the slot site
+      bool left1 = false;               // NEAR-H with ka = 3: the a-vector starts one plane column to the left
+      uint8_t* gpl = nullptr;
+      if (TYPE == PH_FAR) {
+        const int ky = A.phase + 2 * half, kxa = 2 * hi;
+        const int kyb = ky ^ (my & 3), UB = paired ? (U ^ 1) : U, kxb = kxa ^ (mx & 3);
+        const int Xb = X0 ^ ((mx >> 2) & (SEG - 1) & ~15);               // the partner chunk inside the partner tile
+        const int cb = (mx >> 2) & 3;
+        const uint32_t selb = cb == 0 ? 0x3210u : cb == 1 ? 0x2301u : cb == 2 ? 0x1032u : 0x0123u;
+        sgn = A.phase ? -1 : 1;
+        a = ld16(st + off(U, ky, kxa, X0));
+        ea = addf(xsum(U, ky, kxa, X0), addf(ld16(st + off(U, ky - 1, kxa, X0)), ld16(st + off(U, ky + 1, kxa, X0))));
+        b = ld16(st + off(UB, kyb, kxb, Xb));
+        eb = addf(xsum(UB, kyb, kxb, Xb), addf(ld16(st + off(UB, kyb - 1, kxb, Xb)), ld16(st + off(UB, kyb + 1, kxb, Xb))));
+        b = xor_perm<CW>(b, selb); eb = xor_perm<CW>(eb, selb);          // b into a's lane order (lane i <-> i ^ c)
+        y = 4 * Y + ky; kxr = kxa;
+        gpa += kxa * SEG + X0; gpb += kxb * SEG + Xb;
+      } else if (TYPE == PH_NEAR_V) {
+        const int kx = half + 2 * hi, ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3;
+        sgn = ((half + ky) & 1) ? -1 : 1;
+        a = ld16(st + off(U, ky, kx, X0)); b = ld16(st + off(U, ky + 1, kx, X0));     // row 4 = row 0 of the quad below
+        // vertical domino: a's lower neighbour is b, b's upper neighbour is a
+        ea = addf(xsum(U, ky, kx, X0), addf(ld16(st + off(U, ky - 1, kx, X0)), b));
+        eb = addf(xsum(U, ky + 1, kx, X0), addf(a, ld16(st + off(U, ky + 2, kx, X0))));
+        y = 4 * Y + ky; kxr = kx;
+        gpa += kx * SEG + X0; gpb += kx * SEG + X0;
       } else {
-        // ---- NEAR, horizontal dominoes: rows ky = half and half + 2 share ka; lanes are indexed by the b-site ----------
+        // NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site
+        const int ky = half + 2 * hi;
         const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
         const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
         sgn = ((ka + half) & 1) ? -1 : 1;
-        auto ldrow = [&](int kyr, int kx, int sh) -> V16 {
-          V16 v = ld16(st + off(U, kyr, kx, X0));
-          if (sh < 0) v = shift_up(v, st[offL(U, kyr, kx, X0)]);
-          else if (sh > 0) v = shift_down(v, st[offR(U, kyr, kx, X0)]);
-          return v;
-        };
-#pragma unroll
-        for (int v = 0; v < 2; ++v) {
-          const int ky = half + 2 * v, y = 4 * Y + ky;
-          V16 a = ldrow(ky, ka, sh_a), b = ld16(st + off(U, ky, kb, X0));
-          V16 ea = add(add(ldrow(ky, ka + 3, sh_l), b), add(ldrow(ky - 1, ka, sh_a), ldrow(ky + 1, ka, sh_a)));
-          V16 eb = add(add(a, ldrow(ky, kb + 1, sh_r)), add(ld16(st + off(U, ky - 1, kb, X0)), ld16(st + off(U, ky + 1, kb, X0))));
-          // random words: block (c0 = xb>>4, c1 = y), word (xb>>2)&3
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const u32x4 rr = philox4x32_10((uint32_t)(4 * chunkG + j), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-            pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, s_thr, a3);
-          }
-          sigma_sums(a, aF, aT); sigma_sums(b, bF, bT);
-          st16(gpb + 8 * v * SEG + X0, b);                                       // plane row (ky, kb): 8 rows below for v = 1
-          if (sh_a == 0) st16(gpa + 8 * v * SEG + X0, a);
-          else st16_left1_tile(gpa + 8 * v * SEG, reinterpret_cast<uint8_t*>(mp->pl) + 8 * v * SEG, X0, a);
-        }
+        a = ldrow(U, ky, ka, X0, sh_a); b = ld16(st + off(U, ky, kb, X0));
+        ea = addf(addf(ldrow(U, ky, ka + 3, X0, sh_l), b), addf(ldrow(U, ky - 1, ka, X0, sh_a), ldrow(U, ky + 1, ka, X0, sh_a)));
+        eb = addf(addf(a, ldrow(U, ky, kb + 1, X0, sh_r)), addf(ld16(st + off(U, ky - 1, kb, X0)), ld16(st + off(U, ky + 1, kb, X0))));
+        y = 4 * Y + ky; kxr = kb;
+        left1 = sh_a != 0;
+        gpa += 8 * hi * SEG; gpb += 8 * hi * SEG + X0;                           // plane rows (ky, ka), (ky, kb)
+        gpl = reinterpret_cast<uint8_t*>(mp->pl) + 8 * hi * SEG;
       }
+      // everything the item needs is in registers: hand the ring slot back to the producer before the long part
       __syncwarp();
       if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
+      // random words: block c0 = 4*(X>>2) + kx, c1 = y, word X & 3 of the slot site (U3)
+      int a3 = 0;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const u32x4 rr = philox4x32_10((uint32_t)(4 * (4 * chunkG + j) + kxr), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+      }
+      if (TYPE == PH_FAR) {
+        const int cb = (mx >> 2) & 3;
+        const uint32_t selb = cb == 0 ? 0x3210u : cb == 1 ? 0x2301u : cb == 2 ? 0x1032u : 0x0123u;
+        b = xor_perm<CW>(b, selb);
+      }
+      sigma_sums(a, aF, aT); sigma_sums(b, bF, bT);
+      st16(gpb, b);
+      if (TYPE == PH_NEAR_H) { if (!left1) st16(gpa + X0, a); else st16_left1_tile(gpa, gpl, X0, a); }
+      else st16(gpa, a);
       // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
       const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
       const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
       tJ += j11; tV += v11; tn2 += a3;
+      s += ST_GROUPS;                                        // task n + ST_GROUPS lives ST_GROUPS slots further in the ring
+      if (s >= NST) { s -= NST; lap ^= 1; }
     }
     // M and Ms of the sites this thread updated, from their new values: sum sigma = sum f - sum g = (9 accF - accT) / 8.
     // Every site is active in exactly one phase of a sweep, so the two phases add up to the whole lattice (k_fold).

@@ -40,7 +40,7 @@ def test_s1_exact_cover_and_conflict_freeness(L):
             assert (np.diff(ia) > 0).all()
             for t in zip(c0.tolist(), c1.tolist(), wd.tolist()):
                 t = t + (phase,)                                 # the phase is part of the counter (c2 = 2*sweep+phase)
-                assert t not in addr and t[2] < 4 and t[0] < max(L // 16, 1) * 2 and t[1] < L
+                assert t not in addr and t[2] < 4 and t[0] < max(L // 4, 4) and t[1] < L
                 addr.add(t)
             if par[0] == 0:   # FAR: partner by XOR with odd masks, same colour, a-sites at even x
                 mx, my = par[1], par[2]
