@@ -3,10 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C5] [--sweeps-per-step S]
 
-A "step" is one pass of the whole hot path over one batch: S sweeps (default 10) of the configured lattice, each sweep
-= two conflict-free phases of N/4 coupled-pair updates (schedule, loads, Philox, proposal, dE class, acceptance,
-write-back, per-sweep observables and their fp64 accumulation).  Default K=10 steps = the 100 sweeps of BASELINE
-config 5.  One process per GPU; with N > 1 every rank runs its own lattice copy (the path shards over replicas,
+A "step" is one pass of the whole hot path over one batch: S sweeps (default 100 = the whole run of BASELINE config 5)
+of the configured lattice, each sweep = two conflict-free phases of N/4 coupled-pair updates (schedule, loads, Philox,
+proposal, dE class, acceptance, write-back, per-sweep observables and their fp64 accumulation).  One process per GPU; with N > 1 every rank runs its own lattice copy (the path shards over replicas,
 PAPER.md:141; no data-path collective) and the value is the aggregate over ranks ("weak").
 
 Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores.
@@ -31,6 +30,10 @@ METRIC = "coupled-pair updates/ns on 1 B200 and % of HBM roofline (L=16384)"
 UNIT = "pair-updates/ns"
 B_ALG_PER_PAIR = {8: 4.0, 2: 1.0}     # bytes: every site once in, once out per sweep
 B_2PASS_PER_PAIR = {8: 8.0, 2: 2.0}   # two data-dependent phases, each one read + one write of the lattice
+# dram__bytes_read.sum + dram__bytes_write.sum per phase launch from the committed `ncu --set full` capture of this very
+# command (profiles/r01c.md: 268.6 MB read + 95.6 MB written, mean over the FAR / NEAR-H / NEAR-V launches); the
+# algorithmic figure is 268.4 MB, the two-pass floor (read all, write the active half) 402.7 MB
+PROFILED_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 364.2e6}
 
 
 def measured_peaks():
@@ -44,41 +47,75 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """SM clock, power and throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe): NVML polled from
+    a thread every few ms (the timed region is a fraction of a second); nvidia-smi is the fallback."""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.rows, self.reasons, self.stop_flag, self.thread, self.proc, self.nvml = index, [], set(), False, None, None, None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True); self.t.start()
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._poll, daemon=True); self.thread.start()
         except Exception:
-            self.proc = None
+            self.nvml = None
+            try:
+                self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                              "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                self.thread = threading.Thread(target=self._read, daemon=True); self.thread.start()
+            except Exception:
+                self.proc = None
+
+    def _poll(self):
+        n = self.nvml
+        bits = [("hw_slowdown", getattr(n, "nvmlClocksEventReasonHwSlowdown", 0x8)),
+                ("hw_thermal_slowdown", getattr(n, "nvmlClocksEventReasonHwThermalSlowdown", 0x40)),
+                ("sw_thermal_slowdown", getattr(n, "nvmlClocksEventReasonSwThermalSlowdown", 0x20)),
+                ("sw_power_cap", getattr(n, "nvmlClocksEventReasonSwPowerCap", 0x4))]
+        get_reasons = getattr(n, "nvmlDeviceGetCurrentClocksEventReasons", None) or getattr(n, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        while not self.stop_flag:
+            try:
+                mhz = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                pw = n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+                self.rows.append((mhz, pw))
+                r = int(get_reasons(self.handle))
+                for name, bit in bits:
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def _read(self):
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ln in self.proc.stdout:
-            self.rows.append([c.strip() for c in ln.split(",")])
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) >= 7 and c[0].replace(".", "").isdigit():
+                self.rows.append((float(c[0]), float(c[2]) if c[2].replace(".", "").isdigit() else 0.0))
+                self.max_mhz = float(c[1]) if c[1].replace(".", "").isdigit() else None
+                for k, nme in enumerate(names):
+                    if c[3 + k].lower().startswith("active"):
+                        self.reasons.add(nme)
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
-        sm = sorted(float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit())
-        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
-        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for k, n in enumerate(names) if any(len(r) >= 7 and r[3 + k].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+        if self.thread is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no NVML and no nvidia-smi"]}
+        self.stop_flag = True
+        if self.proc:
+            time.sleep(0.05); self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm = sorted(r[0] for r in self.rows)
+        pw = [r[1] for r in self.rows]
+        order = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": getattr(self, "max_mhz", None),
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": [r for r in order if r in self.reasons],
+                "source": "nvml" if self.nvml else "nvidia-smi"}
 
 
 def cpu_oracle_rate(cfg, code, nsweeps, threads):
@@ -115,7 +152,7 @@ def run_reference(args, cfg):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int8 state, uint32 thresholds, fp64 observables", "data": "synthetic",
+        "vs_baseline": None, "dtype": "u8", "data": "synthetic",
         "config": {"workload": f"{args.config}: L={cfg['L']} n={cfg['n']} Delta={cfg['delta']} V={cfg['V']} J={cfg['J']} T={cfg['T'][0]}",
                    "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -131,10 +168,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C5", choices=sorted(ic_inputs.CONFIGS))
-    ap.add_argument("--sweeps-per-step", type=int, default=10)
+    ap.add_argument("--sweeps-per-step", type=int, default=100)
     ap.add_argument("--bits", type=int, default=0, help="override bits per site (8 or 2)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the timed CPU-oracle sample")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     cfg = dict(ic_inputs.CONFIGS[args.config])
@@ -233,7 +271,8 @@ def main():
     pairs_per_launch = reps * N // 4
     ach = B_ALG_PER_PAIR[bits] * pairs_per_launch / (avg_ms * 1e6)
     ach2 = B_2PASS_PER_PAIR[bits] * pairs_per_launch / (avg_ms * 1e6)
-    roofline = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+    roofline = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get((args.config, bits)) if world == 1 and reps == 1 else None,
                 "kernel": "phase kernel (one of the two phases of a sweep)", "avg_launch_ms": avg_ms, "peak_source": peak_src,
                 "bytes_per_pair_algorithmic": B_ALG_PER_PAIR[bits],
                 "two_pass": {"bytes_per_pair": B_2PASS_PER_PAIR[bits], "achieved": ach2, "frac": ach2 / peak}}
@@ -243,8 +282,9 @@ def main():
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": f"{'int8' if bits == 8 else '2-bit'} state, uint32 thresholds, int64/fp64 observables", "data": "synthetic",
-            "config": {"workload": f"{args.config}: L={L} n={cfg['n']} Delta={cfg['delta']} V={cfg['V']} J={cfg['J']} "
+            "dtype": "u8" if bits == 8 else "u2", "data": "synthetic",
+            "config": {"arithmetic": f"{'1 byte' if bits == 8 else '2 bits'} per site, uint32 Philox words and thresholds, int64 / fp64 observables",
+                       "workload": f"{args.config}: L={L} n={cfg['n']} Delta={cfg['delta']} V={cfg['V']} J={cfg['J']} "
                                    f"T={Ts[0]}..{Ts[-1]} x{reps} replica(s), {bits} bits/site, seeded stage-1 state with exact charge {sim.Q}",
                        "sweeps_per_step": S, "pairs_per_step_per_gpu": pairs_per_step, "parallelism": f"replicas x{world}",
                        "l2": f"lattice {reps * N * bits // 8 >> 20} MiB per GPU " + ("> 126 MB L2 (inputs larger than L2, no flush)" if reps * N * bits // 8 > 126e6 else "fits L2 (L2-resident by design)")},
@@ -254,11 +294,11 @@ def main():
             out["e2e"] = e2e
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
-            Ls = min(L, 4096)
+            Ls = min(L, 8192)
             import oracle
             dens = cfg["nplus"] / float(N)
             code = oracle.init_state(Ls, Ls, int(round(dens * Ls * Ls)), 0, cfg["seed"], 0)
-            nsw = 4
+            nsw = max(1, int(args.cpu_seconds * 0.07e9 * min(cores, 16) / 16 / (Ls * Ls // 2)))   # ~0.07 pairs/ns on 16 cores
             v, dt = cpu_oracle_rate(cfg, code, nsw, cores)
             out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                                    "sample": f"{nsw} sweeps of a {Ls}x{Ls} lattice with the workload's parameters and charge density, OpenMP over rows"}
