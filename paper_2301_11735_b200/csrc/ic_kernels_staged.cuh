@@ -95,7 +95,7 @@ __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity)
         : "r"(bar), "r"(parity)
         : "memory");
     if (ok) break;
-    __nanosleep(1000);
+    __nanosleep(100);
   }
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -266,6 +266,18 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
       int Yq[2], sg[2];
 #pragma unroll
       for (int U = 0; U < 2; ++U) { const int rho = region_of(t, U); Yq[U] = rho >> lognseg; sg[U] = rho & (nseg - 1); }
+      // bytes across the tile edge (lane = staged row (ky_rel + 1) * 4 + kx): plain loads, issued first so that their
+      // latency overlaps with the issue of the bulk copies
+      uint8_t hl[2] = {0, 0}, hr[2] = {0, 0};
+      if (hf) {
+        const int kyr = (lane >> 2) - 1, kx = lane & 3, ky = kyr & 3;
+#pragma unroll
+        for (int U = 0; U < 2; ++U) {
+          const int Yr = kyr < 0 ? ((Yq[U] - 1) & Wm) : kyr > 3 ? ((Yq[U] + 1) & Wm) : Yq[U];
+          if (hf & 1) hl[U] = lat[p16_row(lw, ky, kx, Yr, (sg[U] - 1) & (nseg - 1)) + SEG - 1];
+          if (hf & 2) hr[U] = lat[p16_row(lw, ky, kx, Yr, (sg[U] + 1) & (nseg - 1))];
+        }
+      }
       if (lane == 0) {
         mbar_arrive_expect_tx(full, (uint32_t)C::TASK_TX);
 #pragma unroll
@@ -275,36 +287,34 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
           bulk_g2s(dst, lat + p16_row(lw, 3, 0, (Yq[U] - 1) & Wm, sg[U]), 4 * SEG, full);
           bulk_g2s(dst + 20 * SEG, lat + p16_row(lw, 0, 0, (Yq[U] + 1) & Wm, sg[U]), (C::ROWS - 20) * SEG, full);
         }
-        for (int sub = 0; sub < 4; ++sub) {
-          // sub-task (U, half): where its items store to, and the coordinates for the Philox counters
-          const int U = sub >> 1, half = sub & 1, Y = Yq[U], seg = sg[U];
-          SubMeta mt; mt.Y = Y; mt.S0 = seg << LOGSEG; mt.pl = 0ull;
-          if (TYPE == PH_FAR) {
-            const int UP = paired ? (U ^ 1) : U;
-            const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
-            mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
-            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yq[UP], sg[UP]));
-          } else if (TYPE == PH_NEAR_V) {
-            const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-            mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
-            mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yb, seg));
-          } else {
-            const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
-            mt.pa = (unsigned long long)(lat + p16_row(lw, half, ka, Y, seg));
-            mt.pb = (unsigned long long)(lat + p16_row(lw, half, kb, Y, seg));
-            mt.pl = (unsigned long long)(lat + p16_row(lw, half, ka, Y, (seg - 1) & (nseg - 1)) + SEG - 1);
-          }
-          reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA)[sub] = mt;
+      }
+      if (lane >= 28) {
+        // sub-task (U, half): where its items store to, and the coordinates for the Philox counters
+        const int sub = lane - 28, U = sub >> 1, half = sub & 1, Y = Yq[U], seg = sg[U];
+        SubMeta mt; mt.Y = Y; mt.S0 = seg << LOGSEG; mt.pl = 0ull;
+        if (TYPE == PH_FAR) {
+          const int UP = paired ? (U ^ 1) : U;
+          const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
+          mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
+          mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yq[UP], sg[UP]));
+        } else if (TYPE == PH_NEAR_V) {
+          const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
+          mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
+          mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yb, seg));
+        } else {
+          const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
+          mt.pa = (unsigned long long)(lat + p16_row(lw, half, ka, Y, seg));
+          mt.pb = (unsigned long long)(lat + p16_row(lw, half, kb, Y, seg));
+          mt.pl = (unsigned long long)(lat + p16_row(lw, half, ka, Y, (seg - 1) & (nseg - 1)) + SEG - 1);
         }
+        SubMeta* dstm = reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + sub;
+        dstm->pa = mt.pa; dstm->pb = mt.pb; dstm->pl = mt.pl; dstm->Y = mt.Y; dstm->S0 = mt.S0;
       }
       if (hf) {
-        // bytes across the tile edge: lane = staged row (ky_rel + 1) * 4 + kx
-        const int kyr = (lane >> 2) - 1, kx = lane & 3, ky = kyr & 3;
 #pragma unroll
         for (int U = 0; U < 2; ++U) {
-          const int Yr = kyr < 0 ? ((Yq[U] - 1) & Wm) : kyr > 3 ? ((Yq[U] + 1) & Wm) : Yq[U];
-          if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = lat[p16_row(lw, ky, kx, Yr, (sg[U] - 1) & (nseg - 1)) + SEG - 1];
-          if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = lat[p16_row(lw, ky, kx, Yr, (sg[U] + 1) & (nseg - 1))];
+          if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = hl[U];
+          if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = hr[U];
         }
       }
       __syncwarp();
