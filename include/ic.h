@@ -119,8 +119,10 @@ int64_t ic_sweep_count(const ic_ctx* ctx);        /* global sweep counter; -1 if
 int64_t ic_charge(const ic_ctx* ctx);             /* Q = llround(n*N); 0 if ctx is NULL                */
 
 /* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
- * 2 = tiled kernels, 3 = shared-memory-resident multi-sweep kernel.  IC_ERR_PARAM if the variant cannot
- * run this context's (L, bits_per_site).  All variants produce identical lattices.                   */
+ * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels
+ * (8 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default from L = 4096 on).
+ * IC_ERR_PARAM if the variant cannot run this context's (L, bits_per_site).  All variants produce identical
+ * lattices and observables.                                                                           */
 int ic_set_variant(ic_ctx* ctx, int variant);
 
 /* Number of kernels launched by this context since ic_create (for bench.py's gpu_launches).         */
