@@ -225,12 +225,19 @@ static int recompute_into_scratch(ic_ctx* c, int replica) {
 }
 
 // Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.
-static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
+// Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.  `validate`, if given,
+// runs on the host while the copy into the staging buffer is in flight; a non-zero result leaves the lattice untouched.
+template <class F>
+static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, F validate) {
   char* lat = c->lattice + (long long)replica * c->lat_stride;
   if (c->layout == LAY_ROW8) {
+    int v = validate();
+    if (v != IC_OK) return v;
     IC_CUDA(cudaMemcpyAsync(lat, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
   } else {
     IC_CUDA(cudaMemcpyAsync(c->d_stage, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
+    int v = validate();
+    if (v != IC_OK) { cudaStreamSynchronize(c->stream); return v; }   // h_codes is the caller's again
     const long long n16 = c->N / 16;
     const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 16);
     if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
@@ -244,6 +251,9 @@ static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
+}
+static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
+  return upload_state(c, replica, h_codes, [] { return (int)IC_OK; });
 }
 
 extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, double J, uint64_t seed, int replicas,
@@ -338,19 +348,38 @@ extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nm
 extern "C" int ic_set_state(ic_ctx* c, int replica, const int8_t* h_codes) {
   if (!c || !h_codes) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
-  // every code in 0..3 and sum S == Q, eight sites at a time: bit1 = charge, bit0 = sign
-  long long nch = 0, nneg = 0; uint64_t bad = 0;
-  const long long N = c->N;   // N >= 16 and a multiple of 8
-  for (long long i = 0; i < N; i += 8) {
-    uint64_t v; memcpy(&v, h_codes + i, 8);
-    bad |= v & 0xFCFCFCFCFCFCFCFCull;
-    const uint64_t ch = (v >> 1) & 0x0101010101010101ull;
-    nch += __builtin_popcountll(ch);
-    nneg += __builtin_popcountll(ch & v);
-  }
-  if (bad) return IC_ERR_CHARGE;
-  if ((nch - nneg) - nneg != c->Q) return IC_ERR_CHARGE;
-  int rc = upload_state(c, replica, h_codes);
+  // every code in 0..3 and sum S == Q (eq. 2), eight sites at a time: bit1 = charge, bit0 = sign; on several host
+  // threads, while the copy into the staging buffer is under way
+  auto validate = [&]() -> int {
+    const long long N = c->N;   // N >= 16 and a multiple of 8
+    unsigned hw = std::thread::hardware_concurrency();
+    const int nth = N < (1 << 20) ? 1 : (int)std::max(1u, std::min(hw ? hw : 1u, 16u));
+    std::vector<long long> nch(nth, 0), nneg(nth, 0); std::vector<uint64_t> bad(nth, 0);
+    auto scan = [&](int t) {
+      const long long lo = (N / 8 * t / nth) * 8, hi = (N / 8 * (t + 1) / nth) * 8;
+      long long a = 0, b = 0; uint64_t x = 0;
+      for (long long i = lo; i < hi; i += 8) {
+        uint64_t v; memcpy(&v, h_codes + i, 8);
+        x |= v & 0xFCFCFCFCFCFCFCFCull;
+        const uint64_t ch = (v >> 1) & 0x0101010101010101ull;
+        a += __builtin_popcountll(ch);
+        b += __builtin_popcountll(ch & v);
+      }
+      nch[t] = a; nneg[t] = b; bad[t] = x;
+    };
+    if (nth == 1) scan(0);
+    else {
+      std::vector<std::thread> th;
+      for (int t = 0; t < nth; ++t) th.emplace_back(scan, t);
+      for (auto& t : th) t.join();
+    }
+    long long A = 0, B = 0; uint64_t X = 0;
+    for (int t = 0; t < nth; ++t) { A += nch[t]; B += nneg[t]; X |= bad[t]; }
+    if (X) return IC_ERR_CHARGE;
+    if ((A - B) - B != c->Q) return IC_ERR_CHARGE;
+    return IC_OK;
+  };
+  int rc = upload_state(c, replica, h_codes, validate);
   if (rc != IC_OK) return rc;
   IC_CUDA(cudaStreamSynchronize(c->stream));   // h_codes may be pageable and is the caller's to reuse
   return IC_OK;
