@@ -448,7 +448,12 @@ static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
     IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     configured = true;
   }
-  k_staged_phase<TYPE, CW><<<grid, ST_THREADS, C::SMEM_BYTES, c->stream>>>(a);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = dim3(ST_THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = c->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  IC_CUDA(cudaLaunchKernelEx(&cfg, k_staged_phase<TYPE, CW>, a));
   return IC_OK;
 }
 static bool staged_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L >= 4 * ST_SEG; }
@@ -513,8 +518,15 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
       int rc = staged ? launch_phase_staged(c, a) : tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
       if (rc != IC_OK) return rc;
     }
-    k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ,
-                                                               d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr, absolute ? 1 : 0);
+    {
+      long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)((c->replicas + 127) / 128)); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = absolute ? 1 : 0;
+      cfg.attrs = attr; cfg.numAttrs = 1;
+      IC_CUDA(cudaLaunchKernelEx(&cfg, k_fold, c->d_obs, c->replicas, c->delta, c->V, qJ, trow, absolute ? 1 : 0));
+    }
     c->launches++;
     IC_CUDA(cudaGetLastError());
     c->sweep += 1;

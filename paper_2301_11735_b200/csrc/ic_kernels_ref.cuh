@@ -116,6 +116,8 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
 // U5: after a sweep, E = Delta*n2 + V*bV + (J/4)*bJ and the running sums, one thread per
 // replica, IEEE fp64 with one rounding per operation (no FMA contraction: explicit _rn intrinsics).
 __global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row, int absolute) {
+  asm volatile("griddepcontrol.launch_dependents;");   // no-ops unless launched as a programmatic dependent (staged path)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= replicas) return;
   ReplicaObs* o = &obs[r];

@@ -212,6 +212,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
   const uint32_t bar0 = smem_u32(smem + C::OFF_BAR);                    // full[s] at bar0 + 8 s, empty[s] at + 8 (NST + s)
+  // Programmatic dependent launch: the next kernel of the stream may start its blocks as soon as ours leave their SMs;
+  // it fills its tables (which no kernel writes) and then waits for the whole of this grid before touching the lattice.
+  asm volatile("griddepcontrol.launch_dependents;");
   {
     const uint2* src = A.thr + (long long)r * THR_STRIDE;
     uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
@@ -232,6 +235,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
   }
+  asm volatile("griddepcontrol.wait;" ::: "memory");                    // the previous phase / fold kernel is complete
   __syncthreads();
 
   const int lw = A.logL - 2, W = 1 << lw, Wm = W - 1;
