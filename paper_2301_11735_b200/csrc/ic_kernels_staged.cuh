@@ -29,7 +29,7 @@ constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane co
 constexpr int ST_TPG = ST_SEG / 2;            // consumer threads per group: one 16-pair item each per task
 constexpr int ST_THREADS = 32 * ST_NPROD + ST_GROUPS * ST_TPG;
 constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) in global memory: (coefficients, info)
-constexpr int ST_DESC_SMEM = 16 * 8 * 128;    // in shared memory: [compact key][r][lane & 15] x 8 bytes, a private copy per lane
+constexpr int ST_DESC_SMEM = 28 * 8 * 128;    // in shared memory: [key][r][lane & 15] x 8 bytes, a private copy per lane
 
 template <int TYPE>
 struct StagedCfg {
@@ -42,7 +42,7 @@ struct StagedCfg {
   static constexpr int TASK_TX = 2 * (16 + 4 + (ROWS - 20)) * ST_SEG;   // bytes the bulk copies of one task deliver
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
-  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [16][8][16]
+  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [28][8][16]
   static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_SMEM;         // NSTAGE stage buffers
   static constexpr int OFF_BAR = OFF_STAGE + NSTAGE * STAGE_BYTES;  // full[NSTAGE], empty[NSTAGE]
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGE * 8 + 16;
@@ -95,7 +95,7 @@ __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity)
         : "r"(bar), "r"(parity)
         : "memory");
     if (ok) break;
-    __nanosleep(100);
+    __nanosleep(400);
   }
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -143,7 +143,7 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
 // Four coupled pairs (one 32-bit word of site bytes per side).  All table lookups are 4-byte shared loads: the phase
 // kernels are bound by shared-memory wavefronts, and with 4-byte entries the hot entries of each table (sigma-sigma pairs,
 // classes without charged neighbours) fall into distinct banks.
-//   move descriptor [key][r], key = fa | fb<<1 | ga<<2 | gb<<3, r = w & 7 (the table of two-site configurations,
+//   move descriptor [key][r], key = fa | fb<<1 | ga<<3 | gb<<4, r = w & 7 (the table of two-site configurations,
 //   PAPER.md:66-74), 8 bytes, 16 copies so that every lane of a half warp reads its own banks (no conflicts at all):
 //   coef = four int8 coefficients;  info = shared-memory address of the class base in the threshold table (low 16 bits) |
 //   xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
@@ -163,9 +163,8 @@ __device__ __forceinline__ void pairs4(uint32_t& A4, uint32_t& B4, uint32_t EA4,
   const uint32_t u0 = __byte_perm(FB, GB, 0x5140), u1 = __byte_perm(FB, GB, 0x7362);
   const uint32_t W0 = __byte_perm(t0, u0, 0x5410), W1 = __byte_perm(t0, u0, 0x7632);
   const uint32_t W2 = __byte_perm(t1, u1, 0x5410), W3 = __byte_perm(t1, u1, 0x7632);
-  // compact key fa | fb<<1 | ga<<2 | gb<<3, times 4 in each byte; byte i moved to byte 1 is key * 1024 = its table row
-  const uint32_t X2 = (A4 + 2u * B4) << 1;                // per byte: fa<<1 | fb<<2 | ga<<4 | gb<<5
-  const uint32_t KS = (X2 & 0x30303030u) | ((X2 << 1) & 0x0C0C0C0Cu);
+  // key fa | fb<<1 | ga<<3 | gb<<4 (< 28), times 4 in each byte; byte i moved to byte 1 is key * 1024 = its table row
+  const uint32_t KS = 4u * A4 + 8u * B4;
   const uint2 q0 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4404) + ((w0 & 7u) << 7));   // s_desc includes (lane & 15) * 8
   const uint2 q1 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4414) + ((w1 & 7u) << 7));
   const uint2 q2 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4424) + ((w2 & 7u) << 7));
@@ -222,7 +221,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
     uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
     for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_THREADS) {
-      const int kc = k >> 7, rr = (k >> 4) & 7, key = (kc & 3) | ((kc & 12) << 1);
+      const int key = k >> 7, rr = (k >> 4) & 7;               // keys with bit 2 set do not occur: null entries
       uint2 d = __ldg(&dsrc[key * 8 + rr]);
       d.y += smem_u32(smem + C::OFF_THR);       // low 16 bits: shared-memory address of the class base (< 64 KB)
       desc_s[k] = d;
