@@ -341,6 +341,8 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     auto offR = [&](int UU, int kyr, int kx, int Xc) -> int {
       return Xc != SEG - 16 ? off(UU, kyr, kx, Xc) + 16 : C::OFF_HALO + UU * 64 + 32 + ((kyr + 1) << 2) + (kx & 3);
     };
+    // FAR: byte part of the lane permutation i -> i ^ (mx >> 2 & 15) as a PRMT selector (index b -> b ^ (c & 3))
+    const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
     for (int t = blockIdx.x + g * gridDim.x, s = g, lap = 0; t < ntasks; t += ST_GROUPS * gridDim.x) {
       mbar_wait(bar0 + 8 * s, (uint32_t)lap);
       const uint8_t* st = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
@@ -367,8 +369,6 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
         const int ky = A.phase + 2 * half, kxa = 2 * hi;
         const int kyb = ky ^ (my & 3), UB = paired ? (U ^ 1) : U, kxb = kxa ^ (mx & 3);
         const int Xb = X0 ^ ((mx >> 2) & (SEG - 1) & ~15);               // the partner chunk inside the partner tile
-        const int cb = (mx >> 2) & 3;
-        const uint32_t selb = cb == 0 ? 0x3210u : cb == 1 ? 0x2301u : cb == 2 ? 0x1032u : 0x0123u;
         sgn = A.phase ? -1 : 1;
         a = ld16(st + off(U, ky, kxa, X0));
         ea = addf(xsum(U, ky, kxa, X0), addf(ld16(st + off(U, ky - 1, kxa, X0)), ld16(st + off(U, ky + 1, kxa, X0))));
@@ -410,11 +410,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
         const u32x4 rr = philox4x32_10((uint32_t)(4 * (4 * chunkG + j) + kxr), (uint32_t)y, A.c2, c3, A.key0, A.key1);
         pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
       }
-      if (TYPE == PH_FAR) {
-        const int cb = (mx >> 2) & 3;
-        const uint32_t selb = cb == 0 ? 0x3210u : cb == 1 ? 0x2301u : cb == 2 ? 0x1032u : 0x0123u;
-        b = xor_perm<CW>(b, selb);
-      }
+      if (TYPE == PH_FAR) b = xor_perm<CW>(b, selb);
       sigma_sums(a, aF, aT); sigma_sums(b, bF, bT);
       st16(gpb, b);
       if (TYPE == PH_NEAR_H) { if (!left1) st16(gpa + X0, a); else st16_left1_tile(gpa, gpl, X0, a); }
