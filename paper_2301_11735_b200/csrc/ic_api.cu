@@ -17,6 +17,7 @@
 #include "ic_kernels_ref.cuh"
 #include "ic_kernels_p16.cuh"
 #include "ic_kernels_staged.cuh"
+#include "ic_kernels_resident.cuh"
 
 using namespace ic;
 
@@ -501,6 +502,21 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     c->have_T = true;
   }
 
+  // small lattices: all the sweeps in one launch, one block per replica, lattice resident in shared memory
+  if (c->L <= RES_MAX_L && (c->variant == 0 || c->variant == 4)) {
+    ResidentArgs ra;
+    ra.lattice = c->lattice; ra.thr = c->d_thr; ra.obs = c->d_obs; ra.trace = (long long*)d_trace; ra.lat_stride = c->lat_stride;
+    ra.nsweeps = nsweeps; ra.sweep0 = c->sweep; ra.delta = c->delta; ra.V = c->V; ra.quarterJ = 0.25 * c->J;
+    ra.L = c->L; ra.logL = c->logL; ra.replicas = c->replicas; ra.key0 = (uint32_t)c->seed; ra.key1 = (uint32_t)(c->seed >> 32);
+    if (c->layout == LAY_ROW8) k_resident_sweeps<LAY_ROW8><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
+    else if (c->layout == LAY_ROW2) k_resident_sweeps<LAY_ROW2><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
+    else k_resident_sweeps<LAY_P16><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+    c->sweep += (uint64_t)nsweeps;
+    return IC_OK;
+  }
+
   PhaseArgs a;
   a.lattice = c->lattice; a.thr = c->d_thr; a.desc = c->d_desc; a.desc32 = c->d_desc32; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
   a.L = c->L; a.logL = c->logL; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
@@ -613,7 +629,8 @@ extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->lau
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {
   if (!c) return IC_ERR_NULL;
-  if (variant < 0 || variant > 3) return IC_ERR_PARAM;
+  if (variant < 0 || variant > 4) return IC_ERR_PARAM;
+  if (variant == 4 && c->L > RES_MAX_L) return IC_ERR_PARAM;
   if (variant == 2 && !tiled_ok(c)) return IC_ERR_PARAM;
   if (variant == 3 && !staged_ok(c)) return IC_ERR_PARAM;
   c->variant = variant;

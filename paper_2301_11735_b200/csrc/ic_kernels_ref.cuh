@@ -33,83 +33,109 @@ __device__ __forceinline__ void block_accumulate(ReplicaObs* o, int dn2, int dV,
   }
 }
 
+// Lattice accessors for the pair update below: global memory in any layout, or a row-major byte lattice in shared memory.
+template <int LAY>
+struct GlobalLat {
+  LatView v;
+  __device__ __forceinline__ int load(int x, int y) const { return Sites<LAY>::load(v, x, y); }
+  __device__ __forceinline__ void store(int x, int y, int oldc, int newc) const { Sites<LAY>::store(v, x, y, oldc, newc); }
+};
+struct SmemLat {
+  int8_t* s; int logL;
+  __device__ __forceinline__ int load(int x, int y) const { return s[(y << logL) + x]; }
+  __device__ __forceinline__ void store(int x, int y, int, int newc) const { s[(y << logL) + x] = (int8_t)newc; }
+};
+
+// The t-th coupled pair of a phase of schedule S1 (U4), updated as the paper states it:
+// the plain CUDA statement of the method.  thr(class) returns 8*t29 - 1 of the replica.  Adds the accepted move's
+// changes to dn2, dV, dJ, dM, dMs.
+template <class Lat, class Thr>
+__device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL, int type, int p1, int p2, int phase, uint32_t c2,
+                                                uint32_t c3, uint32_t key0, uint32_t key1, const Thr& thr, long long t,
+                                                int& dn2, int& dV, int& dJ, int& dM, int& dMs) {
+  const int mask = L - 1;
+  // --- which pair (schedule S1) and which random word ---------------------------------------------
+  int xa, ya, xb, yb, adj; uint32_t c0, word;
+  if (type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
+    int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
+    xa = 2 * i; ya = 2 * j + phase; xb = xa ^ p1; yb = ya ^ p2; adj = 0;
+    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
+  } else if (p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
+    int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
+    xa = ((p2 + 2 * ((ya + phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
+    c0 = (((uint32_t)xb >> 4) << 2) | ((uint32_t)xb & 3u); word = ((uint32_t)xb >> 2) & 3u;   // addressed by the b-site
+  } else {                           // NEAR, vertical dominoes
+    xa = (int)(t & mask); int jy = (int)(t >> logL);
+    ya = ((p2 + 2 * ((xa + phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
+    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
+  }
+  u32x4 rnd = philox4x32_10(c0, (uint32_t)ya, c2, c3, key0, key1);
+  uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
+
+  // --- proposal: same pair charge q, configuration r of the paper's list ----------
+  const int ca = lat.load(xa, ya), cb = lat.load(xb, yb);
+  const int q = S_of(ca) + S_of(cb);
+  const int rr = (int)(w & 7u);
+  int na = ca, nb = cb;
+  if (q == 0) {
+    // (S+,S-) (S-,S+) (s+,s+) (s-,s-) (s+,s-) (s-,s+); rr = 6,7: nothing proposed
+    switch (rr) {
+      case 0: na = 2; nb = 3; break;
+      case 1: na = 3; nb = 2; break;
+      case 2: na = 0; nb = 0; break;
+      case 3: na = 1; nb = 1; break;
+      case 4: na = 0; nb = 1; break;
+      case 5: na = 1; nb = 0; break;
+      default: na = ca; nb = cb; break;
+    }
+  } else if (q == 1 || q == -1) {
+    const int C = q > 0 ? 2 : 3;     // (C,s+) (C,s-) (s+,C) (s-,C)
+    switch (rr & 3) {
+      case 0: na = C; nb = 0; break;
+      case 1: na = C; nb = 1; break;
+      case 2: na = 0; nb = C; break;
+      default: na = 1; nb = C; break;
+    }
+  }
+  if (na != ca || nb != cb) {
+    // --- neighbour sums over the four slots of a and of b, current lattice ----------
+    const int xl = (xa - 1) & mask, xr = (xa + 1) & mask, yu = (ya - 1) & mask, yd = (ya + 1) & mask;
+    const int c1 = lat.load(xl, ya), c2 = lat.load(xr, ya);
+    const int c3 = lat.load(xa, yu), c4 = lat.load(xa, yd);
+    const int xl2 = (xb - 1) & mask, xr2 = (xb + 1) & mask, yu2 = (yb - 1) & mask, yd2 = (yb + 1) & mask;
+    const int e1 = lat.load(xl2, yb), e2 = lat.load(xr2, yb);
+    const int e3 = lat.load(xb, yu2), e4 = lat.load(xb, yd2);
+    const int nSa = S_of(c1) + S_of(c2) + S_of(c3) + S_of(c4), nGa = sg_of(c1) + sg_of(c2) + sg_of(c3) + sg_of(c4);
+    const int nSb = S_of(e1) + S_of(e2) + S_of(e3) + S_of(e4), nGb = sg_of(e1) + sg_of(e2) + sg_of(e3) + sg_of(e4);
+    // --- dE class: eq. (4) distant / eq. (5) neighbouring sites, spin term as in DESIGN.md G1 ------
+    const int dSa = S_of(na) - S_of(ca), dSb = S_of(nb) - S_of(cb);
+    const int dGa = sg_of(na) - sg_of(ca), dGb = sg_of(nb) - sg_of(cb);
+    const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
+    const int e_v = dSa * nSa + dSb * nSb + adj * dSa * dSb;
+    const int e_j = dGa * nGa + dGb * nGb + adj * dGa * dGb;
+    const uint32_t t8 = thr(class_index(e_d, e_v, e_j));
+    if (w <= t8) {                   // Metropolis min(1, exp(-dE/T)): (w >> 3) < t29, t8 = 8 t29 - 1
+      lat.store(xa, ya, ca, na);
+      lat.store(xb, yb, cb, nb);
+      dn2 += e_d; dV += e_v; dJ += e_j; dM += dGa + dGb;
+      dMs += (((xa + ya) & 1) ? -dGa : dGa) + (((xb + yb) & 1) ? -dGb : dGb);
+    }
+  }
+}
+
 template <int LAY>
 __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
-  const int L = A.L, logL = A.logL, mask = L - 1;
+  const int L = A.L, logL = A.logL;
   const int r = blockIdx.y;
   const long long npairs = ((long long)L * L) >> 2;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const LatView lat{(char*)A.lattice + (long long)r * A.lat_stride, L, logL};
+  const GlobalLat<LAY> lat{LatView{(char*)A.lattice + (long long)r * A.lat_stride, L, logL}};
+  const uint2* thr_r = A.thr + (long long)r * THR_STRIDE;
+  auto thr = [thr_r](int cls) -> uint32_t { return __ldg(&thr_r[cls]).x; };
   int dn2 = 0, dV = 0, dJ = 0, dM = 0, dMs = 0;
-  if (t < npairs) {
-    // --- which pair (schedule S1) and which random word ---------------------------------------------
-    int xa, ya, xb, yb, adj; uint32_t c0, word;
-    if (A.type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
-      int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
-      xa = 2 * i; ya = 2 * j + A.phase; xb = xa ^ A.p1; yb = ya ^ A.p2; adj = 0;
-      c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
-    } else if (A.p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
-      int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
-      xa = ((A.p2 + 2 * ((ya + A.phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
-      c0 = (((uint32_t)xb >> 4) << 2) | ((uint32_t)xb & 3u); word = ((uint32_t)xb >> 2) & 3u;   // addressed by the b-site
-    } else {                           // NEAR, vertical dominoes
-      xa = (int)(t & mask); int jy = (int)(t >> logL);
-      ya = ((A.p2 + 2 * ((xa + A.phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
-      c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
-    }
-    u32x4 rnd = philox4x32_10(c0, (uint32_t)ya, A.c2, (uint32_t)r | (TAG_UPDATE << 28), A.key0, A.key1);
-    uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
-
-    // --- proposal: same pair charge q, configuration r of the paper's list ----------
-    const int ca = Sites<LAY>::load(lat, xa, ya), cb = Sites<LAY>::load(lat, xb, yb);
-    const int q = S_of(ca) + S_of(cb);
-    const int rr = (int)(w & 7u);
-    int na = ca, nb = cb;
-    if (q == 0) {
-      // (S+,S-) (S-,S+) (s+,s+) (s-,s-) (s+,s-) (s-,s+); rr = 6,7: nothing proposed
-      switch (rr) {
-        case 0: na = 2; nb = 3; break;
-        case 1: na = 3; nb = 2; break;
-        case 2: na = 0; nb = 0; break;
-        case 3: na = 1; nb = 1; break;
-        case 4: na = 0; nb = 1; break;
-        case 5: na = 1; nb = 0; break;
-        default: na = ca; nb = cb; break;
-      }
-    } else if (q == 1 || q == -1) {
-      const int C = q > 0 ? 2 : 3;     // (C,s+) (C,s-) (s+,C) (s-,C)
-      switch (rr & 3) {
-        case 0: na = C; nb = 0; break;
-        case 1: na = C; nb = 1; break;
-        case 2: na = 0; nb = C; break;
-        default: na = 1; nb = C; break;
-      }
-    }
-    if (na != ca || nb != cb) {
-      // --- neighbour sums over the four slots of a and of b, current lattice ----------
-      const int xl = (xa - 1) & mask, xr = (xa + 1) & mask, yu = (ya - 1) & mask, yd = (ya + 1) & mask;
-      const int c1 = Sites<LAY>::load(lat, xl, ya), c2 = Sites<LAY>::load(lat, xr, ya);
-      const int c3 = Sites<LAY>::load(lat, xa, yu), c4 = Sites<LAY>::load(lat, xa, yd);
-      const int xl2 = (xb - 1) & mask, xr2 = (xb + 1) & mask, yu2 = (yb - 1) & mask, yd2 = (yb + 1) & mask;
-      const int e1 = Sites<LAY>::load(lat, xl2, yb), e2 = Sites<LAY>::load(lat, xr2, yb);
-      const int e3 = Sites<LAY>::load(lat, xb, yu2), e4 = Sites<LAY>::load(lat, xb, yd2);
-      const int nSa = S_of(c1) + S_of(c2) + S_of(c3) + S_of(c4), nGa = sg_of(c1) + sg_of(c2) + sg_of(c3) + sg_of(c4);
-      const int nSb = S_of(e1) + S_of(e2) + S_of(e3) + S_of(e4), nGb = sg_of(e1) + sg_of(e2) + sg_of(e3) + sg_of(e4);
-      // --- dE class: eq. (4) distant / eq. (5) neighbouring sites, spin term as in DESIGN.md G1 ------
-      const int dSa = S_of(na) - S_of(ca), dSb = S_of(nb) - S_of(cb);
-      const int dGa = sg_of(na) - sg_of(ca), dGb = sg_of(nb) - sg_of(cb);
-      const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
-      const int e_v = dSa * nSa + dSb * nSb + adj * dSa * dSb;
-      const int e_j = dGa * nGa + dGb * nGb + adj * dGa * dGb;
-      const uint32_t t8 = __ldg(&A.thr[(long long)r * THR_STRIDE + class_index(e_d, e_v, e_j)]).x;
-      if (w <= t8) {                   // Metropolis min(1, exp(-dE/T)): (w >> 3) < t29, t8 = 8 t29 - 1
-        Sites<LAY>::store(lat, xa, ya, ca, na);
-        Sites<LAY>::store(lat, xb, yb, cb, nb);
-        dn2 = e_d; dV = e_v; dJ = e_j; dM = dGa + dGb;
-        dMs = (((xa + ya) & 1) ? -dGa : dGa) + (((xb + yb) & 1) ? -dGb : dGb);
-      }
-    }
-  }
+  if (t < npairs)
+    ref_pair_update(lat, L, logL, A.type, A.p1, A.p2, A.phase, A.c2, (uint32_t)r | (TAG_UPDATE << 28), A.key0, A.key1, thr, t,
+                    dn2, dV, dJ, dM, dMs);
   block_accumulate(&A.obs[r], dn2, dV, dJ, dM, dMs);
 }
 

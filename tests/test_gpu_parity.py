@@ -366,3 +366,31 @@ def test_staged_kernels_self_partnered_regions(pkg):
     assert np.array_equal(a.state(0), b.state(0))
     check_against_oracle(a, [lat], [1.2])
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("L,bits,reps", [(4, 8, 2), (8, 2, 3), (16, 8, 5), (32, 2, 2), (64, 8, 3), (64, 2, 2)])
+def test_resident_kernel_equals_reference_kernels(pkg, L, bits, reps):
+    """Variant 4 (one launch for all sweeps, lattice resident in shared memory; the default for L <= 64) against variant 1
+    (one thread per pair, three launches per sweep): lattices, integers, fp64 sums and the per-sweep trace, with the call
+    split in two on one side and a temperature change in between."""
+    seed = 900 + L + bits
+    nplus, nminus = L * L // 8, L * L // 16
+    n = (nplus - nminus) / (L * L)
+    Ts = [0.3, 0.9, 1.7, 2.6, 3.9][:reps]
+    codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
+    a = pkg.Sim(L, n, -0.5, 1.0, 2.0, seed=seed, replicas=reps, bits_per_site=bits); a.set_variant(4)
+    b = pkg.Sim(L, n, -0.5, 1.0, 2.0, seed=seed, replicas=reps, bits_per_site=bits); b.set_variant(1)
+    for r in range(reps):
+        a.set_state(r, codes[r]); b.set_state(r, codes[r])
+    ta = a.sweep_trace(Ts, 37).cpu().numpy()
+    tb = np.concatenate([b.sweep_trace(Ts, 20).cpu().numpy(), b.sweep_trace(Ts, 17).cpu().numpy()])
+    assert np.array_equal(ta, tb)
+    Ts2 = [t + 0.25 for t in Ts]
+    a.sweep(Ts2, 11); b.sweep(Ts2, 11)
+    assert a.sweep_count == b.sweep_count == 48
+    oa, ob = a.observables(), b.observables()
+    for r in range(reps):
+        assert oa[r] == ob[r], (r, oa[r], ob[r])
+        assert np.array_equal(a.state(r), b.state(r))
+        assert list(a.debug_recompute(r)) == [oa[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    a.close(); b.close()
