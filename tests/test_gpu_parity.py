@@ -394,3 +394,17 @@ def test_resident_kernel_equals_reference_kernels(pkg, L, bits, reps):
         assert np.array_equal(a.state(r), b.state(r))
         assert list(a.debug_recompute(r)) == [oa[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     a.close(); b.close()
+
+
+def test_large_lattice_invariants_l32768(pkg):
+    """A lattice beyond BASELINE's sizes (L = 32768, 1 GiB at one byte per site: 8 segments per plane row, 2^19 staged
+    regions): no oracle run at this size, but eq. (2) holds exactly and the incrementally tracked integers equal the full
+    recomputation from eq. (3) after FAR and NEAR sweeps."""
+    L = 32768
+    sim = pkg.Sim(L, 0.05, 0.2, 1.0, 1.0, seed=9)
+    assert sim.Q == int(np.floor(0.05 * L * L + 0.5))
+    sim.sweep(1.0, 4)
+    o = sim.observables()[0]
+    assert o["Q"] == sim.Q and o["nmeas"] == 4
+    assert list(sim.debug_recompute(0)) == [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    sim.close()
