@@ -1,0 +1,37 @@
+"""-m gpu: the temperature-scan driver against the exact 4 x 4 solution -- the paper's own
+verification ("the exact solution was obtained for a 4 x 4 lattice", Fig. 5).  The exact constrained
+canonical averages come from the enumerated density of states under tests/golden (written by oracle/ only)."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import exact
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.mark.parametrize("delta,V,J,Q,Ts", [(0.5, 1.0, 1.0, 4, [0.3, 0.6, 1.0, 2.0, 4.0]), (-0.5, 1.0, 2.0, 0, [0.8, 1.5, 3.0]),
+                                            (0.0, 0.5, 1.0, 2, [0.4, 1.0, 2.5])])
+def test_scan_reproduces_the_exact_4x4_solution(delta, V, J, Q, Ts):
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2301_11735_b200.scan import temperature_scan
+    L, N = 4, 16
+    dos = exact.load_dos(os.path.join(GOLDEN, "dos_4x4.txt"))
+    res = temperature_scan(L, Q / N, delta, V, J, Ts, equil=20000, sweeps=640000, seed=31, bins=64)
+    assert res["Q"] == Q
+    for i, T in enumerate(Ts):
+        ex = exact.averages(dos, Q, delta, V, J, T)
+        C_ex = (ex["E2"] - ex["E"] ** 2) / (N * T * T)
+        chi_u_ex = ex["M2"] / (N * T)            # <M> = 0 by the sigma -> -sigma symmetry of eq. (3)
+        chi_s_ex = ex["Ms2"] / (N * T)
+        assert abs(res["E"][i] - ex["E"]) <= 4.5 * res["E_err"][i] + 1e-9, (T, res["E"][i], ex["E"], res["E_err"][i])
+        assert abs(res["C"][i] - C_ex) <= 4.5 * res["C_err"][i] + 1e-6, (T, res["C"][i], C_ex, res["C_err"][i])
+        assert abs(res["chi_u"][i] - chi_u_ex) <= 4.5 * res["chi_u_err"][i] + 0.02 * chi_u_ex + 1e-6, (T, res["chi_u"][i], chi_u_ex)
+        assert abs(res["chi_s"][i] - chi_s_ex) <= 4.5 * res["chi_s_err"][i] + 0.02 * chi_s_ex + 1e-6, (T, res["chi_s"][i], chi_s_ex)
+        assert abs(res["n2"][i] - ex["n2"]) <= 0.02 * max(1.0, ex["n2"])
+    # with the exact constraint the heat capacity stays finite as T -> 0 (no 1/T^2 divergence)
+    assert np.all(np.isfinite(res["C"])) and res["C"][0] < 1.0
