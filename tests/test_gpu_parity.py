@@ -408,3 +408,27 @@ def test_large_lattice_invariants_l32768(pkg):
     assert o["Q"] == sim.Q and o["nmeas"] == 4
     assert list(sim.debug_recompute(0)) == [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     sim.close()
+
+
+@pytest.mark.parametrize("case", ["self_partnered", "paired_across_segments_only"])
+def test_staged_kernels_rare_far_masks_l4096(pkg, case):
+    """L = 4096 has two staged regions per row quad.  FAR masks with my < 4 keep the partner in the same row quad: with
+    mx < 2048 every region is its own partner, with mx >= 2048 regions pair across the two segments only.  Such masks come
+    up once in a thousand sweeps, so the seed is searched with the oracle's schedule function; the staged kernels are
+    compared with the one-thread-per-pair kernels (themselves checked against the oracle) after a FAR and a NEAR sweep."""
+    L = 4096
+    want_low = case == "self_partnered"
+    seed = next(sd for sd in range(1, 400000)
+                if oracle.schedule_params(L, sd, 0)[2] < 4 and (oracle.schedule_params(L, sd, 0)[1] < 2048) == want_low)
+    typ, mx, my, _ = oracle.schedule_params(L, seed, 0)
+    assert typ == 0 and my < 4 and (mx < 2048) == want_low
+    code = ic_inputs.random_state(L, L * L // 10, L * L // 12, seed)
+    n = (L * L // 10 - L * L // 12) / (L * L)
+    a = pkg.Sim(L, n, 0.5, 1.0, 1.0, seed=seed); a.set_variant(3); a.set_state(0, code)
+    b = pkg.Sim(L, n, 0.5, 1.0, 1.0, seed=seed); b.set_variant(1); b.set_state(0, code)
+    assert tuple(a.schedule(0)) == (typ, mx, my, 0)
+    a.sweep(0.9, 2); b.sweep(0.9, 2)
+    assert np.array_equal(a.state(0), b.state(0))
+    assert a.observables()[0] == b.observables()[0]
+    assert list(a.debug_recompute(0)) == [a.observables()[0][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    a.close(); b.close()
