@@ -120,7 +120,7 @@ int64_t ic_charge(const ic_ctx* ctx);             /* Q = llround(n*N); 0 if ctx 
 
 /* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
  * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels
- * (8 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default from L = 4096 on).
+ * (8 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default there).
  * 4 = resident kernel (L <= 64, any bits_per_site: one block per replica keeps its lattice in shared memory and
  * runs all sweeps of an ic_sweep call in one launch; the default for L <= 64).
  * IC_ERR_PARAM if the variant cannot run this context's (L, bits_per_site).  All variants produce identical

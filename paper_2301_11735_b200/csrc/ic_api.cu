@@ -405,14 +405,25 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
   return IC_OK;
 }
 
+// Launch as a programmatic dependent of the previous kernel of the stream: the kernel may start while that one drains
+// (every phase kernel and the fold call griddepcontrol.wait before they touch anything a kernel writes).
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
   const long long npairs = c->N / 4;
   dim3 grid((unsigned)((npairs + 255) / 256), (unsigned)c->replicas);
-  if (c->layout == LAY_ROW8) k_ref_phase<LAY_ROW8><<<grid, 256, 0, c->stream>>>(a);
-  else if (c->layout == LAY_ROW2) k_ref_phase<LAY_ROW2><<<grid, 256, 0, c->stream>>>(a);
-  else k_ref_phase<LAY_P16><<<grid, 256, 0, c->stream>>>(a);
+  if (c->layout == LAY_ROW8) IC_CUDA(launch_pdl(k_ref_phase<LAY_ROW8>, grid, dim3(256), 0, c->stream, a));
+  else if (c->layout == LAY_ROW2) IC_CUDA(launch_pdl(k_ref_phase<LAY_ROW2>, grid, dim3(256), 0, c->stream, a));
+  else IC_CUDA(launch_pdl(k_ref_phase<LAY_P16>, grid, dim3(256), 0, c->stream, a));
   c->launches++;
-  IC_CUDA(cudaGetLastError());
   return IC_OK;
 }
 
@@ -425,15 +436,15 @@ static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
   if (a.type == 0) {
     a.desc = c->d_desc;
     switch (((a.p1 >> 2) & 15) >> 2) {
-      case 0: k_p16_phase<PH_FAR, 0><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
-      case 1: k_p16_phase<PH_FAR, 1><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
-      case 2: k_p16_phase<PH_FAR, 2><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
-      default: k_p16_phase<PH_FAR, 3><<<grid, P16_THREADS, 0, c->stream>>>(a); break;
+      case 0: IC_CUDA(launch_pdl(k_p16_phase<PH_FAR, 0>, grid, dim3(P16_THREADS), 0, c->stream, a)); break;
+      case 1: IC_CUDA(launch_pdl(k_p16_phase<PH_FAR, 1>, grid, dim3(P16_THREADS), 0, c->stream, a)); break;
+      case 2: IC_CUDA(launch_pdl(k_p16_phase<PH_FAR, 2>, grid, dim3(P16_THREADS), 0, c->stream, a)); break;
+      default: IC_CUDA(launch_pdl(k_p16_phase<PH_FAR, 3>, grid, dim3(P16_THREADS), 0, c->stream, a)); break;
     }
   } else {
     a.desc = c->d_desc + DESC_ENTRIES;
-    if (a.p1 == 0) k_p16_phase<PH_NEAR_H, 0><<<grid, P16_THREADS, 0, c->stream>>>(a);
-    else k_p16_phase<PH_NEAR_V, 0><<<grid, P16_THREADS, 0, c->stream>>>(a);
+    if (a.p1 == 0) IC_CUDA(launch_pdl(k_p16_phase<PH_NEAR_H, 0>, grid, dim3(P16_THREADS), 0, c->stream, a));
+    else IC_CUDA(launch_pdl(k_p16_phase<PH_NEAR_V, 0>, grid, dim3(P16_THREADS), 0, c->stream, a));
   }
   c->launches++;
   IC_CUDA(cudaGetLastError());
@@ -449,12 +460,7 @@ static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
     IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     configured = true;
   }
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = grid; cfg.blockDim = dim3(ST_THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = c->stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  IC_CUDA(cudaLaunchKernelEx(&cfg, k_staged_phase<TYPE, CW>, a));
+  IC_CUDA(launch_pdl(k_staged_phase<TYPE, CW>, grid, dim3(ST_THREADS), (size_t)C::SMEM_BYTES, c->stream, a));
   return IC_OK;
 }
 static bool staged_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L >= 4 * ST_SEG; }
@@ -528,7 +534,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     bool absolute = false;
     for (int phase = 0; phase < 2; ++phase) {
       a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
-      const bool staged = staged_ok(c) && (c->variant == 3 || (c->variant == 0 && c->L > 4 * ST_SEG));
+      const bool staged = staged_ok(c) && (c->variant == 3 || c->variant == 0);
       const bool tiled = tiled_ok(c) && (c->variant == 0 || c->variant == 2);
       absolute = staged;     // the staged kernels report M, Ms of the updated sites instead of their changes
       int rc = staged ? launch_phase_staged(c, a) : tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
@@ -536,12 +542,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     }
     {
       long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr;
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)((c->replicas + 127) / 128)); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
-      cudaLaunchAttribute attr[1];
-      attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = absolute ? 1 : 0;
-      cfg.attrs = attr; cfg.numAttrs = 1;
-      IC_CUDA(cudaLaunchKernelEx(&cfg, k_fold, c->d_obs, c->replicas, c->delta, c->V, qJ, trow, absolute ? 1 : 0));
+      IC_CUDA(launch_pdl(k_fold, dim3((unsigned)((c->replicas + 127) / 128)), dim3(128), 0, c->stream, c->d_obs, c->replicas, c->delta, c->V, qJ, trow, absolute ? 1 : 0));
     }
     c->launches++;
     IC_CUDA(cudaGetLastError());

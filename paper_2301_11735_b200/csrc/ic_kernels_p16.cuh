@@ -135,12 +135,14 @@ __global__ void __launch_bounds__(P16_THREADS) k_p16_phase(PhaseArgs A) {
   __shared__ __align__(16) uint2 s_thr_tab[THR_STRIDE];
   __shared__ __align__(16) uint2 s_desc_tab[DESC_ENTRIES];
   const int r = blockIdx.y;
+  asm volatile("griddepcontrol.launch_dependents;");      // programmatic dependent launch: see launch_pdl (ic_api.cu)
   {
     const uint4* src = reinterpret_cast<const uint4*>(A.thr + (long long)r * THR_STRIDE);
     uint4* dst = reinterpret_cast<uint4*>(s_thr_tab);
     for (int k = threadIdx.x; k < THR_STRIDE / 2; k += P16_THREADS) dst[k] = __ldg(&src[k]);
     if (threadIdx.x < DESC_ENTRIES) s_desc_tab[threadIdx.x] = __ldg(&A.desc[threadIdx.x]);
   }
+  asm volatile("griddepcontrol.wait;" ::: "memory");      // the tables above are written by no kernel
   __syncthreads();
   const char* s_thr = reinterpret_cast<const char*>(s_thr_tab);
   const char* s_desc = reinterpret_cast<const char*>(s_desc_tab);

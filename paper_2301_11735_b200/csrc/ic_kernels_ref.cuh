@@ -125,6 +125,8 @@ __device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL,
 
 template <int LAY>
 __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
+  asm volatile("griddepcontrol.launch_dependents;");      // programmatic dependent launch: see launch_pdl (ic_api.cu)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   const int L = A.L, logL = A.logL;
   const int r = blockIdx.y;
   const long long npairs = ((long long)L * L) >> 2;
