@@ -31,9 +31,9 @@ UNIT = "pair-updates/ns"
 B_ALG_PER_PAIR = {8: 4.0, 2: 1.0}     # bytes: every site once in, once out per sweep
 B_2PASS_PER_PAIR = {8: 8.0, 2: 2.0}   # two data-dependent phases, each one read + one write of the lattice
 # dram__bytes_read.sum + dram__bytes_write.sum per phase launch from the committed `ncu --set full` capture of this very
-# command (profiles/r01d.md: 268.6 MB read + 94.2 MB written, mean over the FAR / NEAR-H / NEAR-V launches); the
+# command (profiles/r01e.md: 268.6 MB read + 94.0 MB written, mean over the FAR / NEAR-H / NEAR-V launches); the
 # algorithmic figure is 268.4 MB, the two-pass floor (read all, write the active half) 402.7 MB
-PROFILED_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 362.8e6}
+PROFILED_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 362.6e6}
 
 
 def measured_peaks():

@@ -8,8 +8,8 @@
 //     edge (the x-1 neighbour of plane 0 is plane 3 one byte to the left) are fetched by the producer's other lanes
 //     with plain loads into a small side array.  Bulk copies cost ~120 cycles of issue each whatever their size
 //     (measured), which is why the layout makes a region three copies and not twenty.
-//   * 16 consumer warps in 4 groups; group g processes tasks g, g+4, ... of the block, task n lives in ring slot
-//     n mod NSTAGE.  A task is two regions = 4096 coupled pairs.  In a FAR phase the two regions are partners under
+//   * 24 consumer warps in 3 groups; group g processes tasks g, g+3, ... of the block and owns two ring slots
+//     (double buffering; a slot goes back to the producer as soon as the item is in registers).  A task is two regions = 4096 coupled pairs.  In a FAR phase the two regions are partners under
 //     (x^mx, y^my): every byte of both is loaded once and all pairs between them are updated.
 //   * consumers read 16-byte vectors from shared memory (conflict-free LDS.128), do the pair updates (byte-SIMD
 //     neighbour sums, move descriptors, dp4a class index, integer acceptance) and store the updated
@@ -38,7 +38,7 @@ struct StagedCfg {
   static constexpr int OFF_HALO = 2 * REGION_BYTES;                 // uint8 [2 regions][left, right][32 rows]
   static constexpr int OFF_SMETA = OFF_HALO + 128;                  // SubMeta[4]
   static constexpr int STAGE_BYTES = OFF_SMETA + 256;
-  static constexpr int NSTAGE = TYPE == PH_NEAR_V ? 6 : 7;
+  static constexpr int NSTAGE = 2 * ST_GROUPS;                       // two ring slots per consumer group (see the kernel)
   static constexpr int TASK_TX = 2 * (16 + 4 + (ROWS - 20)) * ST_SEG;   // bytes the bulk copies of one task deliver
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
@@ -251,7 +251,11 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     const int rho0 = ((t >> hb) << (hb + 1)) | (t & ((1 << hb) - 1));
     return U ? (rho0 ^ Mrho) : rho0;
   };
-  // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n uses ring slot n % NST
+  // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n belongs to consumer group g = n % ST_GROUPS
+  // and is its k-th task, k = n / ST_GROUPS; it lives in slot g + ST_GROUPS * (k & 1) on lap (k >> 1) & 1.  A slot is thus
+  // always drained by the same group and filled by the same producer warp, both in task order, so nobody can wait on a
+  // barrier more than one phase away from its own -- the only case a parity wait gets wrong.  (With slots shared between
+  // groups a group that ran a lap ahead of a slow producer passed the wait on the previous lap's parity.)
   int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
   int aF = 0, aT = 0, bF = 0, bT = 0, sgn = 1;   // sums over the new site bytes of the a- and b-sites (sigma_sums)
 
@@ -259,9 +263,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     // ============================== producer warps: warp p fills the ring slots s with s % ST_NPROD == p ================
     const int p = tid >> 5;
     const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, (lane >> 2) - 1, lane & 3) : 0;   // lane = staged row
-    // a ring slot is always filled by the same producer warp (slot % ST_NPROD), in task order: a parity wait is only
-    // safe for a waiter that is at most one phase ahead of the barrier
-    for (int t = blockIdx.x, s = 0, lap = 0; t < ntasks; t += gridDim.x, lap ^= (s + 1 == NST), s = (s + 1 == NST) ? 0 : s + 1) {
+    // a slot is always filled by the same producer warp (slot % ST_NPROD), in task order
+    for (int t = blockIdx.x, g = 0, k = 0; t < ntasks; t += gridDim.x, k += (g + 1 == ST_GROUPS), g = (g + 1 == ST_GROUPS) ? 0 : g + 1) {
+      const int s = g + ST_GROUPS * (k & 1), lap = (k >> 1) & 1;
       if (s % ST_NPROD != p) continue;
       mbar_wait_backoff(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1));
       unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
@@ -343,7 +347,8 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     };
     // FAR: byte part of the lane permutation i -> i ^ (mx >> 2 & 15) as a PRMT selector (index b -> b ^ (c & 3))
     const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
-    for (int t = blockIdx.x + g * gridDim.x, s = g, lap = 0; t < ntasks; t += ST_GROUPS * gridDim.x) {
+    for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += ST_GROUPS * gridDim.x, ++k) {
+      const int s = g + ST_GROUPS * (k & 1), lap = (k >> 1) & 1;
       mbar_wait(bar0 + 8 * s, (uint32_t)lap);
       const uint8_t* st = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       const SubMeta* mp = reinterpret_cast<const SubMeta*>(st + C::OFF_SMETA) + sub;
@@ -419,8 +424,6 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
       const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
       const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
       tJ += j11; tV += v11; tn2 += a3;
-      s += ST_GROUPS;                                        // task n + ST_GROUPS lives ST_GROUPS slots further in the ring
-      if (s >= NST) { s -= NST; lap ^= 1; }
     }
     // M and Ms of the sites this thread updated, from their new values: sum sigma = sum f - sum g = (9 accF - accT) / 8.
     // Every site is active in exactly one phase of a sweep, so the two phases add up to the whole lattice (k_fold).
