@@ -433,3 +433,17 @@ def test_staged_kernels_rare_far_masks_l4096(pkg, case):
     assert a.observables()[0] == b.observables()[0]
     assert list(a.debug_recompute(0)) == [a.observables()[0][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     a.close(); b.close()
+
+
+def test_staged_kernels_equal_reference_kernels_at_bench_size(pkg):
+    """The launch configuration bench.py times (L = 16384: 8192 tasks per phase over 148 persistent blocks, every ring slot
+    reused ~9 times per launch) against the one-thread-per-pair kernels, lattices compared after every second sweep: a
+    protocol error in the producer/consumer ring shows up here as sporadically wrong row quads."""
+    L = 16384
+    a = pkg.Sim(L, 0.05, 0.2, 1.0, 1.0, seed=5); a.set_variant(3)
+    b = pkg.Sim(L, 0.05, 0.2, 1.0, 1.0, seed=5); b.set_variant(1)
+    for s in range(4):
+        a.sweep(1.0, 2); b.sweep(1.0, 2)
+        assert np.array_equal(a.state(0), b.state(0)), (s, a.schedule(2 * s), a.schedule(2 * s + 1))
+        assert a.observables()[0] == b.observables()[0]
+    a.close(); b.close()
