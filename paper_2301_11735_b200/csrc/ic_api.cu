@@ -514,9 +514,10 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     ra.lattice = c->lattice; ra.thr = c->d_thr; ra.obs = c->d_obs; ra.trace = (long long*)d_trace; ra.lat_stride = c->lat_stride;
     ra.nsweeps = nsweeps; ra.sweep0 = c->sweep; ra.delta = c->delta; ra.V = c->V; ra.quarterJ = 0.25 * c->J;
     ra.L = c->L; ra.logL = c->logL; ra.replicas = c->replicas; ra.key0 = (uint32_t)c->seed; ra.key1 = (uint32_t)(c->seed >> 32);
-    if (c->layout == LAY_ROW8) k_resident_sweeps<LAY_ROW8><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
-    else if (c->layout == LAY_ROW2) k_resident_sweeps<LAY_ROW2><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
-    else k_resident_sweeps<LAY_P16><<<c->replicas, RES_THREADS, 0, c->stream>>>(ra);
+    const int rthreads = (int)std::min<long long>(RES_THREADS, std::max<long long>(64, (c->N / 4 + 31) / 32 * 32));   // one per pair of a phase
+    if (c->layout == LAY_ROW8) k_resident_sweeps<LAY_ROW8><<<c->replicas, rthreads, 0, c->stream>>>(ra);
+    else if (c->layout == LAY_ROW2) k_resident_sweeps<LAY_ROW2><<<c->replicas, rthreads, 0, c->stream>>>(ra);
+    else k_resident_sweeps<LAY_P16><<<c->replicas, rthreads, 0, c->stream>>>(ra);
     c->launches++;
     IC_CUDA(cudaGetLastError());
     c->sweep += (uint64_t)nsweeps;

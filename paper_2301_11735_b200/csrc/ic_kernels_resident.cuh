@@ -14,7 +14,7 @@
 namespace ic {
 
 constexpr int RES_MAX_L = 64;
-constexpr int RES_THREADS = 256;
+constexpr int RES_THREADS = 512;           // at most; the host launches one thread per pair of a phase, 64 <= threads <= 512
 
 struct ResidentArgs {
   void* lattice;                 // [replicas][lat_stride bytes]
@@ -38,8 +38,9 @@ __global__ void __launch_bounds__(RES_THREADS) k_resident_sweeps(ResidentArgs A)
   const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int L = A.L, logL = A.logL, N = L * L, npairs = N >> 2;
   const LatView gv{(char*)A.lattice + (long long)r * A.lat_stride, L, logL};
-  for (int k = tid; k < THR_STRIDE; k += RES_THREADS) s_thr[k] = __ldg(&A.thr[(long long)r * THR_STRIDE + k]).x;
-  for (int i = tid; i < N; i += RES_THREADS) s_code[i] = (int8_t)Sites<LAY>::load(gv, i & (L - 1), i >> logL);
+  const int nthr = (int)blockDim.x;
+  for (int k = tid; k < THR_STRIDE; k += nthr) s_thr[k] = __ldg(&A.thr[(long long)r * THR_STRIDE + k]).x;
+  for (int i = tid; i < N; i += nthr) s_code[i] = (int8_t)Sites<LAY>::load(gv, i & (L - 1), i >> logL);
   ReplicaObs o;
   if (tid == 0) o = A.obs[r];
   const SmemLat lat{s_code, logL};
@@ -60,7 +61,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_resident_sweeps(ResidentArgs A)
     int dn2 = 0, dV = 0, dJ = 0, dM = 0, dMs = 0;
     for (int phase = 0; phase < 2; ++phase) {
       const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
-      for (int t = tid; t < npairs; t += RES_THREADS)
+      for (int t = tid; t < npairs; t += nthr)
         ref_pair_update(lat, L, logL, type, p1, p2, phase, c2, c3, A.key0, A.key1, thr, (long long)t, dn2, dV, dJ, dM, dMs);
       __syncthreads();       // phase 1 reads neighbours written in phase 0
     }
@@ -70,7 +71,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_resident_sweeps(ResidentArgs A)
     if (lane == 0) { s_red[0][warp] = dn2; s_red[1][warp] = dV; s_red[2][warp] = dJ; s_red[3][warp] = dM; s_red[4][warp] = dMs; }
     __syncthreads();
     if (tid == 0) {
-      for (int wv = 0; wv < RES_THREADS / 32; ++wv) {
+      for (int wv = 0; wv < (nthr >> 5); ++wv) {
         o.n2 += s_red[0][wv]; o.bV += s_red[1][wv]; o.bJ += s_red[2][wv]; o.M += s_red[3][wv]; o.Ms += s_red[4][wv];
       }
       // U5, one rounding per operation, the order of k_fold
@@ -92,14 +93,14 @@ __global__ void __launch_bounds__(RES_THREADS) k_resident_sweeps(ResidentArgs A)
   // write the lattice back in its layout
   if (LAY == LAY_ROW2) {
     uint32_t* words = reinterpret_cast<uint32_t*>(gv.base);
-    for (int wi = tid; wi < (N >> 4); wi += RES_THREADS) {
+    for (int wi = tid; wi < (N >> 4); wi += nthr) {
       uint32_t wd = 0;
 #pragma unroll
       for (int k = 0; k < 16; ++k) wd |= (uint32_t)(s_code[16 * wi + k] & 3) << (2 * k);
       words[wi] = wd;
     }
   } else {
-    for (int i = tid; i < N; i += RES_THREADS) Sites<LAY>::store(gv, i & (L - 1), i >> logL, 0, s_code[i]);
+    for (int i = tid; i < N; i += nthr) Sites<LAY>::store(gv, i & (L - 1), i >> logL, 0, s_code[i]);
   }
   if (tid == 0) A.obs[r] = o;
 }
