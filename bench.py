@@ -34,6 +34,9 @@ B_2PASS_PER_PAIR = {8: 8.0, 2: 2.0}   # two data-dependent phases, each one read
 # command (profiles/r01e.md: 268.6 MB read + 94.0 MB written, mean over the FAR / NEAR-H / NEAR-V launches); the
 # algorithmic figure is 268.4 MB, the two-pass floor (read all, write the active half) 402.7 MB
 PROFILED_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 362.6e6}
+# warp instructions per 32 pair updates = lane instructions per pair update of the phase kernels, same capture (mean of the
+# three kernel types); issue peak = 148 SMs x 4 sub-partitions x 32 lanes x SM clock
+PROFILED_INSTR_PER_PAIR = {("C5", 8): 41.3}
 
 
 def measured_peaks():
@@ -277,6 +280,13 @@ def main():
                 "bytes_per_pair_algorithmic": B_ALG_PER_PAIR[bits],
                 "two_pass": {"bytes_per_pair": B_2PASS_PER_PAIR[bits], "achieved": ach2, "frac": ach2 / peak}}
 
+    ipp = PROFILED_INSTR_PER_PAIR.get((args.config, bits)) if world == 1 and reps == 1 else None
+    if ipp:
+        mhz = clocks.get("sm_mhz") or 1965.0
+        issue_peak = 148 * 4 * 32 * mhz * 1e6
+        roofline["issue"] = {"bound": "alu", "what": "the path is bound by instruction issue / the integer ALU pipe, not by HBM",
+                             "achieved": value * 1e9 * ipp, "peak": issue_peak, "unit": "lane-instructions/s",
+                             "frac": value * 1e9 * ipp / issue_peak, "instructions_per_pair": ipp}
     out = None
     if rank == 0:
         out = {
