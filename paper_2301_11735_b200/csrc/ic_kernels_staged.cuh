@@ -1,6 +1,7 @@
 // ic_kernels_staged.cuh -- variant 3: the production sm_100a kernels for L >= 2048 on the tiled layout LAY_P16.
 //
-// One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM:
+// One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM, launched as a programmatic
+// dependent of the previous kernel of the stream (table fill and barrier set-up overlap that kernel's tail):
 //   * 4 producer warps stage "regions" of the lattice in shared memory with 1-D bulk copies (cp.async.bulk, the TMA
 //     engine; completion on an mbarrier).  A region is one tile of the layout (row quad Y, 512 plane columns: 16 plane
 //     rows = 8 KB contiguous in global memory, ONE copy) plus the plane rows of the lattice row above and of the one
@@ -8,9 +9,10 @@
 //     edge (the x-1 neighbour of plane 0 is plane 3 one byte to the left) are fetched by the producer's other lanes
 //     with plain loads into a small side array.  Bulk copies cost ~120 cycles of issue each whatever their size
 //     (measured), which is why the layout makes a region three copies and not twenty.
-//   * 24 consumer warps in 3 groups; group g processes tasks g, g+3, ... of the block and owns two ring slots
-//     (double buffering; a slot goes back to the producer as soon as the item is in registers).  A task is two regions = 4096 coupled pairs.  In a FAR phase the two regions are partners under
-//     (x^mx, y^my): every byte of both is loaded once and all pairs between them are updated.
+//   * 24 consumer warps in 3 groups; group g processes tasks g, g+3, ... of the block and owns two stage slots
+//     (double buffering; a slot goes back to the producer as soon as the items are in registers).  A task is two
+//     regions = 4096 coupled pairs, a thread's item one 16-byte vector = 16 pairs.  In a FAR phase the two regions are
+//     partners under (x^mx, y^my): every byte of both is loaded once and all pairs between them are updated.
 //   * consumers read 16-byte vectors from shared memory (conflict-free LDS.128), do the pair updates (byte-SIMD
 //     neighbour sums, move descriptors, dp4a class index, integer acceptance) and store the updated
 //     vectors straight to global memory (128-bit stores).
