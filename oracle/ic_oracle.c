@@ -76,10 +76,11 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 
 /* Counter layout:
  *   ctr = (c0, c1, c2, replica | tag<<28),   key = (seed lo, seed hi)          */
+/* tags 0..3 here; oracle/ic_variants.c uses 4..7 */
 enum { TAG_UPDATE = 0, TAG_SCHED = 1, TAG_INIT = 2, TAG_S0 = 3 };
 
-static void philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2,
-                          uint32_t replica, uint32_t tag, uint32_t out[4]) {
+void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2,
+                       uint32_t replica, uint32_t tag, uint32_t out[4]) {
   uint32_t ctr[4] = {c0, c1, c2, (replica & 0x0FFFFFFFu) | (tag << 28)};
   uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
   orc_philox4x32_10(ctr, key, out);
@@ -268,7 +269,7 @@ void orc_init_state(int8_t* code, int Lx, int Ly, int64_t nplus, int64_t nminus,
   int64_t N = (int64_t)Lx * Ly, K = nplus + nminus, picked = 0, plus = 0;
   for (int64_t i = 0; i < N; ++i) {
     uint32_t w[4];
-    philox_tagged(seed, (uint32_t)(i & 0xFFFFFFFF), (uint32_t)(i >> 32), 0, (uint32_t)replica, TAG_INIT, w);
+    orc_philox_tagged(seed, (uint32_t)(i & 0xFFFFFFFF), (uint32_t)(i >> 32), 0, (uint32_t)replica, TAG_INIT, w);
     int c = (w[0] & 1u) ? C_SM : C_SP;
     if ((int64_t)(((uint64_t)w[1] * (uint64_t)(N - i)) >> 32) < (K - picked)) {
       if ((int64_t)(((uint64_t)w[2] * (uint64_t)(K - picked)) >> 32) < (nplus - plus)) { c = C_CP; ++plus; }
@@ -288,7 +289,7 @@ void orc_attach(orc_state* st, const int8_t* code) {
 /* ------------------------------------------------------------------------- */
 /* U5: measurement after a sweep                              */
 /* ------------------------------------------------------------------------- */
-static void measure(orc_state* st, int64_t* trace_row) {
+void orc_measure(orc_state* st, int64_t* trace_row) {
   double E = (st->delta * (double)st->n2 + st->V * (double)st->bV) + (0.25 * st->J) * (double)st->bJ;
   double M = (double)st->M, Ms = (double)st->Ms;
   st->sumE += E; st->sumE2 += E * E;
@@ -317,7 +318,7 @@ void orc_reset_observables(orc_state* st) {
  *   odd  s -> NEAR sweep: o = z0 & 1 (0 horizontal, 1 vertical), off = z1 & 3 */
 void orc_schedule_params(int L, uint64_t seed, uint64_t sweep, int32_t out4[4]) {
   uint32_t z[4];
-  philox_tagged(seed, 0, 0, (uint32_t)sweep, 0, TAG_SCHED, z);
+  orc_philox_tagged(seed, 0, 0, (uint32_t)sweep, 0, TAG_SCHED, z);
   if ((sweep & 1) == 0) {
     out4[0] = 0;
     out4[1] = (int32_t)(2 * (z[0] & (uint32_t)(L / 2 - 1)) + 1);
@@ -400,13 +401,13 @@ int orc_sweep_s1(orc_state* st, int8_t* code, double T, int64_t nsweeps, int ord
           int x = order ? L - 1 - xx : xx;
           int xb, yb; uint32_t c0, c1, word, w[4];
           if (!s1_pair_at(L, par, phase, x, y, &xb, &yb, &c0, &c1, &word)) continue;
-          philox_tagged(st->seed, c0, c1, (uint32_t)(2 * st->sweep + (uint64_t)phase),
+          orc_philox_tagged(st->seed, c0, c1, (uint32_t)(2 * st->sweep + (uint64_t)phase),
                         (uint32_t)st->replica, TAG_UPDATE, w);
           orc_pair_update(st, code, x, y, xb, yb, w[word], T);
         }
       }
     }
-    measure(st, trace ? trace + 6 * s : NULL);
+    orc_measure(st, trace ? trace + 6 * s : NULL);
     st->sweep += 1;
   }
   return 0;
@@ -436,7 +437,7 @@ int orc_sweep_s1_mt(orc_state* st, int8_t* code, double T, int64_t nsweeps, int 
         for (int x = 0; x < L; ++x) {
           int xb, yb; uint32_t c0, c1, word, w[4];
           if (!s1_pair_at(L, par, phase, x, y, &xb, &yb, &c0, &c1, &word)) continue;
-          philox_tagged(st->seed, c0, c1, (uint32_t)(2 * st->sweep + (uint64_t)phase),
+          orc_philox_tagged(st->seed, c0, c1, (uint32_t)(2 * st->sweep + (uint64_t)phase),
                         (uint32_t)st->replica, TAG_UPDATE, w);
           orc_pair_update(&loc, code, x, y, xb, yb, w[word], T);
         }
@@ -446,7 +447,7 @@ int orc_sweep_s1_mt(orc_state* st, int8_t* code, double T, int64_t nsweeps, int 
       st->n2 += d_n2; st->bV += d_bV; st->bJ += d_bJ; st->M += d_M; st->Ms += d_Ms;
       st->n_attempt += d_att; st->n_accept += d_acc; st->n_null += d_null;
     }
-    measure(st, trace ? trace + 6 * s : NULL);
+    orc_measure(st, trace ? trace + 6 * s : NULL);
     st->sweep += 1;
   }
   return 0;
@@ -462,13 +463,13 @@ int orc_sweep_s0(orc_state* st, int8_t* code, double T, int64_t nsweeps, int64_t
   for (int64_t s = 0; s < nsweeps; ++s) {
     for (int64_t k = 0; k < N / 2; ++k) {
       uint32_t w[4];
-      philox_tagged(st->seed, (uint32_t)k, 0, (uint32_t)st->sweep, (uint32_t)st->replica, TAG_S0, w);
+      orc_philox_tagged(st->seed, (uint32_t)k, 0, (uint32_t)st->sweep, (uint32_t)st->replica, TAG_S0, w);
       int64_t a = (int64_t)(((uint64_t)w[2] * (uint64_t)N) >> 32);
       int64_t b = (int64_t)(((uint64_t)w[3] * (uint64_t)(N - 1)) >> 32);
       if (b >= a) ++b;
       orc_pair_update(st, code, (int)(a % st->Lx), (int)(a / st->Lx), (int)(b % st->Lx), (int)(b / st->Lx), w[0], T);
     }
-    measure(st, trace ? trace + 6 * s : NULL);
+    orc_measure(st, trace ? trace + 6 * s : NULL);
     st->sweep += 1;
   }
   return 0;

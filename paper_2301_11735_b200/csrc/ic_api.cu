@@ -35,7 +35,7 @@ struct ic_ctx {
   cudaEvent_t thr_copied;
   std::vector<double>* lastT; bool have_T;
   long long launches;
-  int sm_count;
+  int sm_count, device;
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -216,7 +216,7 @@ __global__ void k_store_ints(ReplicaObs* o, const long long* s8) {
 static int recompute_into_scratch(ic_ctx* c, int replica) {
   IC_CUDA(cudaMemsetAsync(c->d_scratch8, 0, 64, c->stream));
   const LatView lat{c->lattice + (long long)replica * c->lat_stride, c->L, c->logL};
-  const int blocks = (int)std::min<long long>((c->N + 255) / 256, 148 * 8);
+  const int blocks = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);
   if (c->layout == LAY_ROW8) k_recompute<LAY_ROW8><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
   else if (c->layout == LAY_ROW2) k_recompute<LAY_ROW2><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
   else k_recompute<LAY_P16><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
@@ -240,7 +240,7 @@ static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, F validat
     int v = validate();
     if (v != IC_OK) { cudaStreamSynchronize(c->stream); return v; }   // h_codes is the caller's again
     const long long n16 = c->N / 16;
-    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 16);
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
     if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
     else k_codes_to_p16<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint8_t*)lat, c->logL);
     c->launches++;
@@ -306,7 +306,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
       return fail(cuda_fail(cudaGetLastError(), "cudaDeviceGetAttribute(multiProcessorCount)"));
-    c->sm_count = sms;
+    c->sm_count = sms; c->device = dev;
   }
 
   // stage 1 for every replica
@@ -394,7 +394,7 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
     IC_CUDA(cudaMemcpyAsync(h_out, lat, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
   } else {
     const long long n16 = c->N / 16;
-    const int blocks = (int)std::min<long long>((n16 + 255) / 256, 148 * 16);
+    const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
     if (c->layout == LAY_ROW2) k_unpack2<<<blocks, 256, 0, c->stream>>>((const uint32_t*)lat, c->d_stage, n16);
     else k_p16_to_codes<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
     c->launches++;
@@ -431,7 +431,7 @@ static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
 static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
   const long long n_items = c->N / 128;
   const long long nb = (n_items + P16_THREADS - 1) / P16_THREADS;
-  const long long cap = std::max<long long>(1, (148LL * 6 + c->replicas - 1) / c->replicas);
+  const long long cap = std::max<long long>(1, ((long long)c->sm_count * 6 + c->replicas - 1) / c->replicas);
   dim3 grid((unsigned)std::min(nb, cap), (unsigned)c->replicas);
   if (a.type == 0) {
     a.desc = c->d_desc;
@@ -455,10 +455,10 @@ static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
 template <int TYPE, int CW>
 static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
   using C = StagedCfg<TYPE>;
-  static bool configured = false;   // per instantiation
-  if (!configured) {
+  static bool configured[64] = {};   // per instantiation and per device: the attribute belongs to the device's copy of the kernel
+  if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
     IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-    configured = true;
+    if (c->device >= 0 && c->device < 64) configured[c->device] = true;
   }
   IC_CUDA(launch_pdl(k_staged_phase<TYPE, CW>, grid, dim3(ST_THREADS), (size_t)C::SMEM_BYTES, c->stream, a));
   return IC_OK;
@@ -470,6 +470,13 @@ static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
   const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
   dim3 grid((unsigned)std::min(ntasks, cap), (unsigned)c->replicas);
   a.desc32 = c->d_desc32;
+  // Philox: the ten round keys and the parts of the first two rounds that are the same for the whole launch (U3)
+  for (int i = 0; i < 10; ++i) { a.rk[2 * i] = a.key0 + (uint32_t)i * PHILOX_W0; a.rk[2 * i + 1] = a.key1 + (uint32_t)i * PHILOX_W1; }
+  {
+    uint32_t h, l;
+    mulhilo(PHILOX_M1, a.c2, h, l);
+    a.f0 = h ^ a.rk[0]; a.f1 = l; a.f2 = l ^ a.rk[2];
+  }
   int rc;
   if (a.type == 0) {
     switch (((a.p1 >> 2) & 15) >> 2) {

@@ -53,7 +53,8 @@ IC_HD int sg_of(int c) { return (c & 2) ? 0 : 1 - 2 * (c & 1); }
 //   ROW2  2 bits per site, public code, 16 sites per 32-bit word, row-major       (2 bits/site)
 //   P16   one byte per site, tiled: the lattice is cut into tiles of 4 rows x 4*SEGL columns (SEGL = min(L/4, 512));
 //         a tile is stored contiguously as 16 "plane rows" [y&3][x&3] of SEGL bytes (plane column X = x>>2 inside the
-//         tile), tiles in the order [y>>2][X / SEGL].  Byte e = f | g<<3 with (f,g) = sigma+ (1,0), sigma- (0,1),
+//         tile), tiles in the order [X / SEGL][y>>2]: the tiles above and below a tile are its neighbours in memory, so
+//         a tile with the plane rows of the lattice row above and below is ONE contiguous piece (one bulk copy).  Byte e = f | g<<3 with (f,g) = sigma+ (1,0), sigma- (0,1),
 //         S+ (1,1), S- (0,0), so that the byte-wise sum of the four neighbour bytes is F | G<<3 with
 //         sum S = F+G-4,  sum sigma = F-G                                          (8 bits/site, L >= 64)
 // Every phase of schedule S1 updates whole plane rows of P16, so the kernels work on dense 16-byte vectors, and a
@@ -69,7 +70,7 @@ constexpr int P16_LOGSEG_MAX = 9;
 IC_HD int p16_logseg(int lw) { return lw < P16_LOGSEG_MAX ? lw : P16_LOGSEG_MAX; }
 IC_HD long long p16_row(int lw, int ky, int kx, int Y, int seg) {
   const int ls = p16_logseg(lw);
-  return ((((long long)Y << (lw - ls)) + seg) * 16 + (ky * 4 + kx)) << ls;
+  return ((((long long)seg << lw) + Y) * 16 + (ky * 4 + kx)) << ls;
 }
 IC_HD long long p16_site(int lw, int x, int y) {
   const int ls = p16_logseg(lw), X = x >> 2;
@@ -133,6 +134,9 @@ struct PhaseArgs {
   int phase;                     // 0 or 1
   uint32_t c2;                   // 2*sweep + phase
   uint32_t key0, key1;           // Philox key = seed
+  // staged kernels: the ten round keys (key + i * Weyl constants) and the launch-constant parts of the first two rounds
+  uint32_t rk[20];
+  uint32_t f0, f1, f2;           // hi(M1*c2) ^ rk[0];  lo(M1*c2);  lo(M1*c2) ^ rk[2]
 };
 
 }  // namespace ic

@@ -2,15 +2,15 @@
 //
 // One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM, launched as a programmatic
 // dependent of the previous kernel of the stream (table fill and barrier set-up overlap that kernel's tail):
-//   * 4 producer warps stage "regions" of the lattice in shared memory with 1-D bulk copies (cp.async.bulk, the TMA
-//     engine; completion on an mbarrier).  A region is one tile of the layout (row quad Y, 512 plane columns: 16 plane
-//     rows = 8 KB contiguous in global memory, ONE copy) plus the plane rows of the lattice row above and of the one
-//     (NEAR-V: two) below (2 KB / 4 KB contiguous, one copy each).  The few bytes read across the left/right tile
-//     edge (the x-1 neighbour of plane 0 is plane 3 one byte to the left) are fetched by the producer's other lanes
-//     with plain loads into a small side array.  Bulk copies cost ~120 cycles of issue each whatever their size
-//     (measured), which is why the layout makes a region three copies and not twenty.
+//   * 2 producer warps (the last two of the block), one per region of a task, stage "regions" of the lattice in shared
+//     memory with 1-D bulk copies (cp.async.bulk, the TMA engine; completion on an mbarrier).  A region is one tile of
+//     the layout (row quad Y, 512 plane columns: 16 plane rows) plus the plane rows of the lattice row above and of the one
+//     (NEAR-V: two) below.  Tiles are stored in the order [segment][Y], so the whole region is ONE contiguous piece of
+//     12 KB (NEAR-V: 14 KB) and one bulk copy (two at the periodic wrap Y = 0 / Y = W-1).  The few bytes read across the
+//     left/right tile edge (the x-1 neighbour of plane 0 is plane 3 one byte to the left) are fetched by the producer's
+//     lanes with plain loads, issued a task ahead, into a small side array.
 //   * 24 consumer warps in 3 groups; group g processes tasks g, g+3, ... of the block and owns two stage slots
-//     (double buffering; a slot goes back to the producer as soon as the items are in registers).  A task is two
+//     (double buffering; a slot goes back to the producers as soon as the items are in registers).  A task is two
 //     regions = 4096 coupled pairs, a thread's item one 16-byte vector = 16 pairs.  In a FAR phase the two regions are
 //     partners under (x^mx, y^my): every byte of both is loaded once and all pairs between them are updated.
 //   * consumers read 16-byte vectors from shared memory (conflict-free LDS.128), do the pair updates (byte-SIMD
@@ -26,12 +26,22 @@
 namespace ic {
 
 constexpr int ST_GROUPS = 3;                  // consumer groups per block
-constexpr int ST_NPROD = 4;                   // producer warps per block
+constexpr int ST_NPROD = 2;                   // producer warps per block: one per region of a task
 constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane columns per region = per tile of the layout
 constexpr int ST_TPG = ST_SEG / 2;            // consumer threads per group: one 16-pair item each per task
-constexpr int ST_THREADS = 32 * ST_NPROD + ST_GROUPS * ST_TPG;
+constexpr int ST_CONS = ST_GROUPS * ST_TPG;   // consumer threads (warps 0..23); the producers are warps 24, 25
+constexpr int ST_THREADS = ST_CONS + 32 * ST_NPROD;
 constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) in global memory: (coefficients, info)
 constexpr int ST_DESC_SMEM = 28 * 8 * 128;    // in shared memory: [key][r][lane & 15] x 8 bytes, a private copy per lane
+
+// What the consumers of one sub-task (region U, half) need to know about the task in a stage.
+struct SubMeta {
+  unsigned long long pa;     // global address of the a-side plane row (see the consumers)
+  unsigned long long pb;     // global address of the b-side plane row
+  unsigned long long pl;     // NEAR-H: address of the byte left of the a-side plane row (last byte of the tile to the left)
+  int Y, C0;                 // row quad and first 16-column chunk of the sub-task's region (Philox counters)
+};
+static_assert(sizeof(SubMeta) == 32, "SubMeta layout");
 
 template <int TYPE>
 struct StagedCfg {
@@ -39,9 +49,8 @@ struct StagedCfg {
   static constexpr int REGION_BYTES = ROWS * ST_SEG;
   static constexpr int OFF_HALO = 2 * REGION_BYTES;                 // uint8 [2 regions][left, right][32 rows]
   static constexpr int OFF_SMETA = OFF_HALO + 128;                  // SubMeta[4]
-  static constexpr int STAGE_BYTES = OFF_SMETA + 256;
-  static constexpr int NSTAGE = 2 * ST_GROUPS;                       // two ring slots per consumer group (see the kernel)
-  static constexpr int TASK_TX = 2 * (16 + 4 + (ROWS - 20)) * ST_SEG;   // bytes the bulk copies of one task deliver
+  static constexpr int STAGE_BYTES = OFF_SMETA + 128;
+  static constexpr int NSTAGE = 2 * ST_GROUPS;                      // slots 2g, 2g+1 belong to consumer group g
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
   static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [28][8][16]
@@ -49,16 +58,6 @@ struct StagedCfg {
   static constexpr int OFF_BAR = OFF_STAGE + NSTAGE * STAGE_BYTES;  // full[NSTAGE], empty[NSTAGE]
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGE * 8 + 16;
 };
-
-// What the consumers of one sub-task (region U, half) need to know about the task in a stage.
-struct SubMeta {
-  unsigned long long pa;     // global address of the a-side plane row (see the consumers)
-  unsigned long long pb;     // global address of the b-side plane row
-  unsigned long long pl;     // NEAR-H: address of the byte left of the a-side plane row (last byte of the tile to the left)
-  int Y, S0;                 // row quad and first plane column of the sub-task's region (Philox counters)
-  int pad[8];
-};
-static_assert(sizeof(SubMeta) == 64, "SubMeta layout");
 
 // ---------------------------------------------------------------------------------------------------------------
 // PTX helpers: mbarrier and 1-D bulk copy global -> shared (TMA engine).
@@ -70,34 +69,20 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+// try_wait suspends the thread in hardware up to the time hint (ns): a waiter costs a handful of instructions per wake-up
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, uint32_t hint_ns) {
   uint32_t ok = 0;
   while (!ok) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok)
-        : "r"(bar), "r"(parity)
+        : "r"(bar), "r"(parity), "r"(hint_ns)
         : "memory");
-  }
-}
-// producers are far ahead of the consumers most of the time: sleep between polls instead of burning issue slots
-__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
-  uint32_t ok = 0;
-  while (true) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    if (ok) break;
-    __nanosleep(400);
   }
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -105,15 +90,25 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                "l"(src), "r"(bytes), "r"(bar)
                : "memory");
 }
-// read-only tables in shared memory: plain (non-volatile) asm so that the compiler may schedule them freely
-__device__ __forceinline__ uint4 lds_tab128(uint32_t addr) {
-  uint4 v;
-  asm("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+// staged lattice bytes: volatile (ordered with the barrier operations); tables: plain asm, free to schedule
+__device__ __forceinline__ V16 lds_v16(uint32_t addr) {
+  V16 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.w[0]), "=r"(v.w[1]), "=r"(v.w[2]), "=r"(v.w[3]) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
   return v;
 }
 __device__ __forceinline__ uint2 lds_tab64(uint32_t addr) {
   uint2 v;
   asm("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_tab32(uint32_t addr) {
+  uint32_t v;
+  asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
 
@@ -141,6 +136,28 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
   return f;
 }
 
+// Philox4x32-10 with the round keys precomputed on the host (PhaseArgs::rk) and the launch-constant parts of the first two
+// rounds folded: counter (c0, y, c2, c3), key (k0, k1).  x0 = f0 ^ y and cb = c3 ^ rk[1] are formed once per item / block.
+struct PhiloxItem { uint32_t x0, hi0, lo0; };   // x0 = c0' of round 1 (the same for the four blocks of an item), M0 * x0
+__device__ __forceinline__ u32x4 philox_staged(uint32_t c0, const PhiloxItem& it, uint32_t cb, const PhaseArgs& A) {
+  // round 0: (c0, y, c2, c3) -> (hi(M1 c2) ^ y ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0))
+  uint32_t h, l;
+  mulhilo(PHILOX_M0, c0, h, l);
+  uint32_t x2 = h ^ cb, x3 = l;
+  // round 1: x0 = it.x0, x1 = f1
+  uint32_t h1, l1;
+  mulhilo(PHILOX_M1, x2, h1, l1);
+  uint32_t y0 = h1 ^ A.f2, y1 = l1, y2 = it.hi0 ^ x3 ^ A.rk[3], y3 = it.lo0;
+#pragma unroll
+  for (int round = 2; round < 10; ++round) {
+    uint32_t a, b, c, d;
+    mulhilo(PHILOX_M0, y0, a, b);
+    mulhilo(PHILOX_M1, y2, c, d);
+    y0 = c ^ y1 ^ A.rk[2 * round]; y1 = d; y2 = a ^ y3 ^ A.rk[2 * round + 1]; y3 = b;
+  }
+  u32x4 r; r.v[0] = y0; r.v[1] = y1; r.v[2] = y2; r.v[3] = y3; return r;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Four coupled pairs (one 32-bit word of site bytes per side).  All table lookups are 4-byte shared loads: the phase
 // kernels are bound by shared-memory wavefronts, and with 4-byte entries the hot entries of each table (sigma-sigma pairs,
@@ -151,11 +168,6 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
 //   xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
 //   class tables [class]: threshold 8*t29 - 1 (accept iff w <= it), packed (dn2, dV, dJ).
 // ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t lds_tab32(uint32_t addr) {
-  uint32_t v;
-  asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-  return v;
-}
 __device__ __forceinline__ void pairs4(uint32_t& A4, uint32_t& B4, uint32_t EA4, uint32_t EB4, uint32_t w0, uint32_t w1,
                                        uint32_t w2, uint32_t w3, uint32_t s_desc, int& a3) {
   // neighbour sums as (4F, 8G), G coefficients halved: the dp4a below yields a byte address in the 4-byte thresholds
@@ -204,15 +216,17 @@ __device__ __forceinline__ void st16_left1_tile(uint8_t* row, uint8_t* left, int
 
 // ---------------------------------------------------------------------------------------------------------------
 // The phase kernel.  TYPE: PH_FAR / PH_NEAR_H / PH_NEAR_V; CW: word part of the FAR lane permutation.
-// grid = (blocks, replicas), block = 4 producer warps + 4 groups of 128 consumer threads.
+// grid = (blocks, replicas), block = 3 groups of 256 consumer threads + 2 producer warps.
 // ---------------------------------------------------------------------------------------------------------------
 template <int TYPE, int CW>
-__global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
+__global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_constant__ PhaseArgs A) {
   using C = StagedCfg<TYPE>;
   constexpr int SEG = ST_SEG, LOGSEG = ST_LOGSEG, NST = C::NSTAGE;
   extern __shared__ __align__(128) unsigned char smem[];
   const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
-  const uint32_t bar0 = smem_u32(smem + C::OFF_BAR);                    // full[s] at bar0 + 8 s, empty[s] at + 8 (NST + s)
+  const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);               // warp-uniform for the compiler
+  const uint32_t smem0 = smem_u32(smem);
+  const uint32_t bar0 = smem0 + C::OFF_BAR;                             // full[s] at bar0 + 8 s, empty[s] at + 8 (NST + s)
   // Programmatic dependent launch: the next kernel of the stream may start its blocks as soon as ours leave their SMs;
   // it fills its tables (which no kernel writes) and then waits for the whole of this grid before touching the lattice.
   asm volatile("griddepcontrol.launch_dependents;");
@@ -225,12 +239,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_THREADS) {
       const int key = k >> 7, rr = (k >> 4) & 7;               // keys with bit 2 set do not occur: null entries
       uint2 d = __ldg(&dsrc[key * 8 + rr]);
-      d.y += smem_u32(smem + C::OFF_THR);       // low 16 bits: shared-memory address of the class base (< 64 KB)
+      d.y += smem0 + C::OFF_THR;                // low 16 bits: shared-memory address of the class base (< 64 KB)
       desc_s[k] = d;
     }
     if (tid == 0) {
       for (int s = 0; s < NST; ++s) {
-        mbar_init(bar0 + 8 * s, 2);                                     // producer lane 0: expect_tx, and after the edge bytes
+        mbar_init(bar0 + 8 * s, ST_NPROD);                              // one arrival per producer warp (+ the bytes of its copies)
         mbar_init(bar0 + 8 * (NST + s), ST_TPG / 32);                   // the warps of the consuming group
       }
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -253,91 +267,87 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     const int rho0 = ((t >> hb) << (hb + 1)) | (t & ((1 << hb) - 1));
     return U ? (rho0 ^ Mrho) : rho0;
   };
+  // byte offset of the tile (Y, seg) in the lattice: tiles in the order [seg][Y], 16 plane rows of SEG bytes each
+  auto tile_off = [&](int Y, int seg) -> long long { return (((long long)seg << lw) + Y) << (LOGSEG + 4); };
   // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n belongs to consumer group g = n % ST_GROUPS
-  // and is its k-th task, k = n / ST_GROUPS; it lives in slot g + ST_GROUPS * (k & 1) on lap (k >> 1) & 1.  A slot is thus
-  // always drained by the same group and filled by the same producer warp, both in task order, so nobody can wait on a
-  // barrier more than one phase away from its own -- the only case a parity wait gets wrong.  (With slots shared between
-  // groups a group that ran a lap ahead of a slow producer passed the wait on the previous lap's parity.)
+  // and is its k-th task, k = n / ST_GROUPS; it lives in slot 2 g + (k & 1) on lap (k >> 1) & 1.  A slot is thus always
+  // drained by the same group and filled in task order, so nobody can wait on a barrier more than one phase away from
+  // its own -- the only case a parity wait gets wrong.
   int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
   int aF = 0, aT = 0, bF = 0, bT = 0, sgn = 1;   // sums over the new site bytes of the a- and b-sites (sigma_sums)
 
-  if (tid < 32 * ST_NPROD) {
-    // ============================== producer warps: warp p fills the ring slots s with s % ST_NPROD == p ================
-    const int p = tid >> 5;
-    const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, (lane >> 2) - 1, lane & 3) : 0;   // lane = staged row
-    // a slot is always filled by the same producer warp (slot % ST_NPROD), in task order
-    for (int t = blockIdx.x, g = 0, k = 0; t < ntasks; t += gridDim.x, k += (g + 1 == ST_GROUPS), g = (g + 1 == ST_GROUPS) ? 0 : g + 1) {
-      const int s = g + ST_GROUPS * (k & 1), lap = (k >> 1) & 1;
-      if (s % ST_NPROD != p) continue;
-      mbar_wait_backoff(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1));
-      unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
+  if (warp >= ST_CONS / 32) {
+    // ============================== producer warp U: region U of every task of the block ================================
+    const int U = warp - ST_CONS / 32;
+    const int kyr = (lane >> 2) - 1, kx = lane & 3;                     // lane = staged row (ky_rel + 1) * 4 + kx
+    const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, kyr, kx) : 0;
+    const int dY = kyr < 0 ? -1 : kyr > 3 ? 1 : 0;
+    const int rowoff = (((kyr & 3) << 2) | kx) << LOGSEG;
+    // the edge bytes of a task are loaded one task ahead (their latency hides behind the wait for the ring slot)
+    auto halo_load = [&](int t, uint32_t& hl, uint32_t& hr) {
+      hl = 0u; hr = 0u;
+      if (hf && t < ntasks) {
+        const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1), Yr = (Yq + dY) & Wm;
+        if (hf & 1) hl = lat[tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + SEG - 1];
+        if (hf & 2) hr = lat[tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff];
+      }
+    };
+    uint32_t hl, hr;
+    halo_load((int)blockIdx.x, hl, hr);
+    for (int t = blockIdx.x, g = 0, k = 0; t < ntasks; t += gridDim.x) {
+      const int s = 2 * g + (k & 1), lap = (k >> 1) & 1;
       const uint32_t full = bar0 + 8 * s;
-      int Yq[2], sg[2];
-#pragma unroll
-      for (int U = 0; U < 2; ++U) { const int rho = region_of(t, U); Yq[U] = rho >> lognseg; sg[U] = rho & (nseg - 1); }
-      // bytes across the tile edge (lane = staged row (ky_rel + 1) * 4 + kx): plain loads, issued first so that their
-      // latency overlaps with the issue of the bulk copies
-      uint8_t hl[2] = {0, 0}, hr[2] = {0, 0};
-      if (hf) {
-        const int kyr = (lane >> 2) - 1, kx = lane & 3, ky = kyr & 3;
-#pragma unroll
-        for (int U = 0; U < 2; ++U) {
-          const int Yr = kyr < 0 ? ((Yq[U] - 1) & Wm) : kyr > 3 ? ((Yq[U] + 1) & Wm) : Yq[U];
-          if (hf & 1) hl[U] = lat[p16_row(lw, ky, kx, Yr, (sg[U] - 1) & (nseg - 1)) + SEG - 1];
-          if (hf & 2) hr[U] = lat[p16_row(lw, ky, kx, Yr, (sg[U] + 1) & (nseg - 1))];
-        }
-      }
+      const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1);
+      mbar_wait(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1), 20000u);
+      unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       if (lane == 0) {
-        mbar_arrive_expect_tx(full, (uint32_t)C::TASK_TX);
-#pragma unroll
-        for (int U = 0; U < 2; ++U) {
-          const uint32_t dst = smem_u32(stg + U * C::REGION_BYTES);
-          bulk_g2s(dst + 4 * SEG, lat + p16_row(lw, 0, 0, Yq[U], sg[U]), 16 * SEG, full);
-          bulk_g2s(dst, lat + p16_row(lw, 3, 0, (Yq[U] - 1) & Wm, sg[U]), 4 * SEG, full);
-          bulk_g2s(dst + 20 * SEG, lat + p16_row(lw, 0, 0, (Yq[U] + 1) & Wm, sg[U]), (C::ROWS - 20) * SEG, full);
+        mbar_expect_tx(full, (uint32_t)C::REGION_BYTES);
+        const uint32_t dst = smem_u32(stg + U * C::REGION_BYTES);
+        if (Yq != 0 && Yq != Wm) {
+          bulk_g2s(dst, lat + tile_off(Yq - 1, sg) + 12 * SEG, C::REGION_BYTES, full);
+        } else if (Yq == 0) {
+          bulk_g2s(dst, lat + tile_off(Wm, sg) + 12 * SEG, 4 * SEG, full);
+          bulk_g2s(dst + 4 * SEG, lat + tile_off(0, sg), (C::ROWS - 4) * SEG, full);
+        } else {
+          bulk_g2s(dst, lat + tile_off(Yq - 1, sg) + 12 * SEG, 20 * SEG, full);
+          bulk_g2s(dst + 20 * SEG, lat + tile_off(0, sg), (C::ROWS - 20) * SEG, full);
         }
       }
-      if (lane >= 28) {
+      if (lane >= 30) {
         // sub-task (U, half): where its items store to, and the coordinates for the Philox counters
-        const int sub = lane - 28, U = sub >> 1, half = sub & 1, Y = Yq[U], seg = sg[U];
-        SubMeta mt; mt.Y = Y; mt.S0 = seg << LOGSEG; mt.pl = 0ull;
+        const int half = lane & 1;
+        SubMeta mt; mt.Y = Yq; mt.C0 = sg << (LOGSEG - 4); mt.pl = 0ull;
         if (TYPE == PH_FAR) {
-          const int UP = paired ? (U ^ 1) : U;
+          const int rhoP = paired ? (rho ^ Mrho) : rho;
           const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
-          mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
-          mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yq[UP], sg[UP]));
+          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((ky * 4) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(rhoP >> lognseg, rhoP & (nseg - 1)) + ((kyb * 4) << LOGSEG));
         } else if (TYPE == PH_NEAR_V) {
-          const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-          mt.pa = (unsigned long long)(lat + p16_row(lw, ky, 0, Y, seg));
-          mt.pb = (unsigned long long)(lat + p16_row(lw, kyb, 0, Yb, seg));
+          const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Yq + (ky == 3)) & Wm;
+          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((ky * 4) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(Yb, sg) + ((kyb * 4) << LOGSEG));
         } else {
           const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
-          mt.pa = (unsigned long long)(lat + p16_row(lw, half, ka, Y, seg));
-          mt.pb = (unsigned long long)(lat + p16_row(lw, half, kb, Y, seg));
-          mt.pl = (unsigned long long)(lat + p16_row(lw, half, ka, Y, (seg - 1) & (nseg - 1)) + SEG - 1);
+          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((half * 4 + ka) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(Yq, sg) + ((half * 4 + kb) << LOGSEG));
+          mt.pl = (unsigned long long)(lat + tile_off(Yq, (sg - 1) & (nseg - 1)) + ((half * 4 + ka) << LOGSEG) + SEG - 1);
         }
-        SubMeta* dstm = reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + sub;
-        dstm->pa = mt.pa; dstm->pb = mt.pb; dstm->pl = mt.pl; dstm->Y = mt.Y; dstm->S0 = mt.S0;
+        *(reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + 2 * U + half) = mt;
       }
-      if (hf) {
-#pragma unroll
-        for (int U = 0; U < 2; ++U) {
-          if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = hl[U];
-          if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = hr[U];
-        }
-      }
+      if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = (uint8_t)hl;
+      if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = (uint8_t)hr;
+      halo_load(t + (int)gridDim.x, hl, hr);
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
+      if (++g == ST_GROUPS) { g = 0; ++k; }
     }
   } else {
     // =========================================== consumer warps ====================================================
-    const int ct = tid - 32 * ST_NPROD, g = ct / ST_TPG, tg = ct - g * ST_TPG;
     // item = one 16-byte vector of a-sites (b-sites for NEAR-H) = 16 coupled pairs: sub-task (U, half), plane/row selector
-    // hi, chunk of 16 plane columns (SEG / 16 = 32 chunks); all but the chunk are uniform in a warp
-    const int sub = tg >> 6, hi = (tg >> 5) & 1, chunk = tg & 31, U = sub >> 1, half = sub & 1, X0 = chunk << 4;
-    const uint32_t s_desc = smem_u32(smem + C::OFF_DESC) + (uint32_t)(lane & 15) * 8u;
-    const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
-    auto addf = [](const V16& p, const V16& q) -> V16 { return add(p, q); };
+    // hi, chunk of 16 plane columns (SEG / 16 = 32 chunks = the lanes of a warp); all but the chunk are uniform in a warp
+    const int g = warp >> 3, wg = warp & 7, sub = wg >> 1, hi = wg & 1, chunk = lane, U = sub >> 1, half = sub & 1, X0 = chunk << 4;
+    const uint32_t s_desc = smem0 + C::OFF_DESC + (uint32_t)(lane & 15) * 8u;
+    const uint32_t cb = ((uint32_t)r | (TAG_UPDATE << 28)) ^ A.rk[1];
     // byte offsets inside a stage buffer: the 16 bytes at plane column Xc of staged row (ky_rel, kx) of region UU,
     // and the bytes just left / right of them (across the tile edge: the side array filled by the producer)
     auto off = [&](int UU, int kyr, int kx, int Xc) -> int { return UU * C::REGION_BYTES + ((((kyr + 1) << 2) + (kx & 3)) << LOGSEG) + Xc; };
@@ -347,74 +357,109 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(PhaseArgs A) {
     auto offR = [&](int UU, int kyr, int kx, int Xc) -> int {
       return Xc != SEG - 16 ? off(UU, kyr, kx, Xc) + 16 : C::OFF_HALO + UU * 64 + 32 + ((kyr + 1) << 2) + (kx & 3);
     };
-    // FAR: byte part of the lane permutation i -> i ^ (mx >> 2 & 15) as a PRMT selector (index b -> b ^ (c & 3))
-    const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
+    // ---- thread-constant offsets of everything the item loads (relative to the stage buffer) --------------------------
+    // o[0] a, o[1] b, o[2..] neighbour vectors; h[..] bytes across the vector's edge for the shifted loads
+    int oa, ob, on[4], oh[4], kxr, ky_ctr;
+    int sh_a = 0, sh_l = 0, sh_r = 0;
+    uint32_t selb = 0x3210u;
+    int goffa, goffb;                          // byte offsets of the item's stores from SubMeta::pa / pb
+    bool left1 = false;
+    if (TYPE == PH_FAR) {
+      const int ky = A.phase + 2 * half, kxa = 2 * hi;
+      const int kyb = ky ^ (my & 3), UB = paired ? (U ^ 1) : U, kxb = kxa ^ (mx & 3);
+      const int Xb = X0 ^ ((mx >> 2) & (SEG - 1) & ~15);               // the partner chunk inside the partner tile
+      sgn = A.phase ? -1 : 1;
+      oa = off(U, ky, kxa, X0); ob = off(UB, kyb, kxb, Xb);
+      on[0] = off(U, ky, kxa + 3, X0); on[1] = off(U, ky, kxa + 1, X0);          // left (shifted if kxa == 0), right of a
+      on[2] = off(UB, kyb, kxb + 3, Xb); on[3] = off(UB, kyb, kxb + 1, Xb);      // left, right (shifted if kxb == 3) of b
+      oh[0] = offL(U, ky, kxa + 3, X0); oh[1] = offR(UB, kyb, kxb + 1, Xb); oh[2] = oh[3] = 0;
+      sh_l = kxa == 0; sh_r = kxb == 3;
+      selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));          // byte part of the lane permutation i -> i ^ (mx >> 2 & 15)
+      ky_ctr = ky; kxr = kxa;
+      goffa = kxa * SEG + X0; goffb = kxb * SEG + Xb;
+    } else if (TYPE == PH_NEAR_V) {
+      const int kx = half + 2 * hi, ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3;
+      sgn = ((half + ky) & 1) ? -1 : 1;
+      oa = off(U, ky, kx, X0); ob = off(U, ky + 1, kx, X0);            // row 4 = row 0 of the quad below
+      on[0] = off(U, ky, kx + 3, X0); on[1] = off(U, ky, kx + 1, X0);
+      on[2] = off(U, ky + 1, kx + 3, X0); on[3] = off(U, ky + 1, kx + 1, X0);
+      sh_l = kx == 0; sh_r = kx == 3;
+      oh[0] = sh_l ? offL(U, ky, kx + 3, X0) : offR(U, ky, kx + 1, X0);
+      oh[1] = sh_l ? offL(U, ky + 1, kx + 3, X0) : offR(U, ky + 1, kx + 1, X0);
+      oh[2] = oh[3] = 0;
+      ky_ctr = ky; kxr = kx;
+      goffa = kx * SEG + X0; goffb = kx * SEG + X0;
+    } else {
+      // NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site
+      const int ky = half + 2 * hi;
+      const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
+      sh_a = ka == 3; sh_l = sh_a || ka == 0; sh_r = kb == 3;
+      sgn = ((ka + half) & 1) ? -1 : 1;
+      oa = off(U, ky, ka, X0); ob = off(U, ky, kb, X0);
+      on[0] = off(U, ky, ka + 3, X0); on[1] = off(U, ky, kb + 1, X0);            // left of a, right of b
+      on[2] = 0; on[3] = 0;
+      oh[0] = offL(U, ky, ka, X0);                                               // a, a-up, a-down: +- 4 rows from here
+      oh[1] = offL(U, ky, ka + 3, X0); oh[2] = offR(U, ky, kb + 1, X0); oh[3] = 0;
+      ky_ctr = ky; kxr = kb;
+      left1 = sh_a != 0;
+      goffa = 8 * hi * SEG; goffb = 8 * hi * SEG + X0;                 // plane rows (ky, ka), (ky, kb)
+    }
+    constexpr int ROW4 = 4 << LOGSEG;                                  // four staged rows = one lattice row up / down
+    const uint32_t stg_g = smem0 + C::OFF_STAGE + 2 * g * C::STAGE_BYTES;
+    const SubMeta* meta_g = reinterpret_cast<const SubMeta*>(smem + C::OFF_STAGE + 2 * g * C::STAGE_BYTES + C::OFF_SMETA) + sub;
+
     for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += ST_GROUPS * gridDim.x, ++k) {
-      const int s = g + ST_GROUPS * (k & 1), lap = (k >> 1) & 1;
-      mbar_wait(bar0 + 8 * s, (uint32_t)lap);
-      const uint8_t* st = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
-      const SubMeta* mp = reinterpret_cast<const SubMeta*>(st + C::OFF_SMETA) + sub;
-      const int Y = mp->Y, chunkG = (mp->S0 >> 4) + chunk;
-      uint8_t* gpa = reinterpret_cast<uint8_t*>(mp->pa);
-      uint8_t* gpb = reinterpret_cast<uint8_t*>(mp->pb);
-      // the 16 bytes of plane kx at row kyr, shifted by one site to the left (sh < 0) or right (sh > 0) if asked
-      auto ldrow = [&](int UU, int kyr, int kx, int Xc, int sh) -> V16 {
-        V16 v = ld16(st + off(UU, kyr, kx, Xc));
-        if (sh < 0) v = shift_up(v, st[offL(UU, kyr, kx, Xc)]);
-        else if (sh > 0) v = shift_down(v, st[offR(UU, kyr, kx, Xc)]);
-        return v;
-      };
-      // left + right neighbours of the vector of plane kx: planes kx-1 and kx+1, one site over when they wrap around
-      auto xsum = [&](int UU, int kyr, int kx, int Xc) -> V16 {
-        return addf(ldrow(UU, kyr, kx + 3, Xc, kx == 0 ? -1 : 0), ldrow(UU, kyr, kx + 1, Xc, kx == 3 ? 1 : 0));
-      };
-      V16 a, b, ea, eb;
-      int y, kxr;                       // Philox counters: lattice row and plane of the slot site
-      bool left1 = false;               // NEAR-H with ka = 3: the a-vector starts one plane column to the left
+      const int s = 2 * g + (k & 1), lap = (k >> 1) & 1;
+      const uint32_t st = stg_g + (k & 1) * C::STAGE_BYTES;
+      mbar_wait(bar0 + 8 * s, (uint32_t)lap, 1000u);
+      const SubMeta* mp = reinterpret_cast<const SubMeta*>(reinterpret_cast<const unsigned char*>(meta_g) + (k & 1) * C::STAGE_BYTES);
+      const int Y = mp->Y, chunkG = mp->C0 + chunk;
+      uint8_t* gpa = reinterpret_cast<uint8_t*>(mp->pa) + goffa;
+      uint8_t* gpb = reinterpret_cast<uint8_t*>(mp->pb) + goffb;
       uint8_t* gpl = nullptr;
+      V16 a, b, ea, eb;
       if (TYPE == PH_FAR) {
-        const int ky = A.phase + 2 * half, kxa = 2 * hi;
-        const int kyb = ky ^ (my & 3), UB = paired ? (U ^ 1) : U, kxb = kxa ^ (mx & 3);
-        const int Xb = X0 ^ ((mx >> 2) & (SEG - 1) & ~15);               // the partner chunk inside the partner tile
-        sgn = A.phase ? -1 : 1;
-        a = ld16(st + off(U, ky, kxa, X0));
-        ea = addf(xsum(U, ky, kxa, X0), addf(ld16(st + off(U, ky - 1, kxa, X0)), ld16(st + off(U, ky + 1, kxa, X0))));
-        b = ld16(st + off(UB, kyb, kxb, Xb));
-        eb = addf(xsum(UB, kyb, kxb, Xb), addf(ld16(st + off(UB, kyb - 1, kxb, Xb)), ld16(st + off(UB, kyb + 1, kxb, Xb))));
+        a = lds_v16(st + oa); b = lds_v16(st + ob);
+        V16 l = lds_v16(st + on[0]);
+        if (sh_l) l = shift_up(l, lds_u8(st + oh[0]));
+        ea = add(add(l, lds_v16(st + on[1])), add(lds_v16(st + oa - ROW4), lds_v16(st + oa + ROW4)));
+        V16 rr = lds_v16(st + on[3]);
+        if (sh_r) rr = shift_down(rr, lds_u8(st + oh[1]));
+        eb = add(add(lds_v16(st + on[2]), rr), add(lds_v16(st + ob - ROW4), lds_v16(st + ob + ROW4)));
         b = xor_perm<CW>(b, selb); eb = xor_perm<CW>(eb, selb);          // b into a's lane order (lane i <-> i ^ c)
-        y = 4 * Y + ky; kxr = kxa;
-        gpa += kxa * SEG + X0; gpb += kxb * SEG + Xb;
       } else if (TYPE == PH_NEAR_V) {
-        const int kx = half + 2 * hi, ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3;
-        sgn = ((half + ky) & 1) ? -1 : 1;
-        a = ld16(st + off(U, ky, kx, X0)); b = ld16(st + off(U, ky + 1, kx, X0));     // row 4 = row 0 of the quad below
+        a = lds_v16(st + oa); b = lds_v16(st + ob);
+        V16 al = lds_v16(st + on[0]), ar = lds_v16(st + on[1]), bl = lds_v16(st + on[2]), br = lds_v16(st + on[3]);
+        if (sh_l) { al = shift_up(al, lds_u8(st + oh[0])); bl = shift_up(bl, lds_u8(st + oh[1])); }
+        if (sh_r) { ar = shift_down(ar, lds_u8(st + oh[0])); br = shift_down(br, lds_u8(st + oh[1])); }
         // vertical domino: a's lower neighbour is b, b's upper neighbour is a
-        ea = addf(xsum(U, ky, kx, X0), addf(ld16(st + off(U, ky - 1, kx, X0)), b));
-        eb = addf(xsum(U, ky + 1, kx, X0), addf(a, ld16(st + off(U, ky + 2, kx, X0))));
-        y = 4 * Y + ky; kxr = kx;
-        gpa += kx * SEG + X0; gpb += kx * SEG + X0;
+        ea = add(add(al, ar), add(lds_v16(st + oa - ROW4), b));
+        eb = add(add(bl, br), add(a, lds_v16(st + ob + ROW4)));
       } else {
-        // NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site
-        const int ky = half + 2 * hi;
-        const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
-        const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
-        sgn = ((ka + half) & 1) ? -1 : 1;
-        a = ldrow(U, ky, ka, X0, sh_a); b = ld16(st + off(U, ky, kb, X0));
-        ea = addf(addf(ldrow(U, ky, ka + 3, X0, sh_l), b), addf(ldrow(U, ky - 1, ka, X0, sh_a), ldrow(U, ky + 1, ka, X0, sh_a)));
-        eb = addf(addf(a, ldrow(U, ky, kb + 1, X0, sh_r)), addf(ld16(st + off(U, ky - 1, kb, X0)), ld16(st + off(U, ky + 1, kb, X0))));
-        y = 4 * Y + ky; kxr = kb;
-        left1 = sh_a != 0;
-        gpa += 8 * hi * SEG; gpb += 8 * hi * SEG + X0;                           // plane rows (ky, ka), (ky, kb)
-        gpl = reinterpret_cast<uint8_t*>(mp->pl) + 8 * hi * SEG;
+        a = lds_v16(st + oa); b = lds_v16(st + ob);
+        V16 au = lds_v16(st + oa - ROW4), ad = lds_v16(st + oa + ROW4), al = lds_v16(st + on[0]), br = lds_v16(st + on[1]);
+        if (sh_a) {
+          a = shift_up(a, lds_u8(st + oh[0]));
+          au = shift_up(au, lds_u8(st + oh[0] + (X0 ? -ROW4 : -4))); ad = shift_up(ad, lds_u8(st + oh[0] + (X0 ? ROW4 : 4)));
+        }
+        if (sh_l) al = shift_up(al, lds_u8(st + oh[1]));
+        if (sh_r) br = shift_down(br, lds_u8(st + oh[2]));
+        ea = add(add(al, b), add(au, ad));
+        eb = add(add(a, br), add(lds_v16(st + ob - ROW4), lds_v16(st + ob + ROW4)));
+        gpl = reinterpret_cast<uint8_t*>(mp->pl) + goffa;
       }
-      // everything the item needs is in registers: hand the ring slot back to the producer before the long part
+      // everything the item needs is in registers: hand the ring slot back to the producers before the long part
       __syncwarp();
       if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
       // random words: block c0 = 4*(X>>2) + kx, c1 = y, word X & 3 of the slot site (U3)
+      PhiloxItem it;
+      it.x0 = A.f0 ^ (uint32_t)(4 * Y + ky_ctr);
+      mulhilo(PHILOX_M0, it.x0, it.hi0, it.lo0);
+      const uint32_t c0base = (uint32_t)(16 * chunkG + kxr);
       int a3 = 0;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        const u32x4 rr = philox4x32_10((uint32_t)(4 * (4 * chunkG + j) + kxr), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        const u32x4 rr = philox_staged(c0base + 4u * j, it, cb, A);
         pairs4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
       }
       if (TYPE == PH_FAR) b = xor_perm<CW>(b, selb);
