@@ -2,7 +2,7 @@
 //
 // One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM, launched as a programmatic
 // dependent of the previous kernel of the stream (table fill and barrier set-up overlap that kernel's tail):
-//   * 2 producer warps (the last two of the block), one per region of a task, stage "regions" of the lattice in shared
+//   * 3 producer warps (the last three of the block), one per consumer group, stage "regions" of the lattice in shared
 //     memory with 1-D bulk copies (cp.async.bulk, the TMA engine; completion on an mbarrier).  A region is one tile of
 //     the layout (row quad Y, 512 plane columns: 16 plane rows) plus the plane rows of the lattice row above and of the one
 //     (NEAR-V: two) below.  Tiles are stored in the order [segment][Y], so the whole region is ONE contiguous piece of
@@ -26,13 +26,14 @@
 namespace ic {
 
 constexpr int ST_GROUPS = 3;                  // consumer groups per block
-constexpr int ST_NPROD = 2;                   // producer warps per block: one per region of a task
+constexpr int ST_NPROD = ST_GROUPS;           // producer warps per block: one per consumer group
 constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane columns per region = per tile of the layout
 constexpr int ST_TPG = ST_SEG / 2;            // consumer threads per group: one 16-pair item each per task
-constexpr int ST_CONS = ST_GROUPS * ST_TPG;   // consumer threads (warps 0..23); the producers are warps 24, 25
+constexpr int ST_CONS = ST_GROUPS * ST_TPG;   // consumer threads (warps 0..23); the producers are warps 24..26
 constexpr int ST_THREADS = ST_CONS + 32 * ST_NPROD;
 constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) in global memory: (coefficients, info)
-constexpr int ST_DESC_SMEM = 28 * 8 * 128;    // in shared memory: [key][r][lane & 15] x 8 bytes, a private copy per lane
+constexpr int ST_DESC_SMEM = 28 * 8 * 128;    // in shared memory: [r][key][lane & 15] x 8 bytes, a private copy per lane
+constexpr uint32_t ST_DESC_RSTRIDE = 28 * 128;
 
 // What the consumers of one sub-task (region U, half) need to know about the task in a stage.
 struct SubMeta {
@@ -53,7 +54,7 @@ struct StagedCfg {
   static constexpr int NSTAGE = 2 * ST_GROUPS;                      // slots 2g, 2g+1 belong to consumer group g
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
-  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [28][8][16]
+  static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [8][28][16]
   static constexpr int OFF_STAGE = OFF_DESC + ST_DESC_SMEM;         // NSTAGE stage buffers
   static constexpr int OFF_BAR = OFF_STAGE + NSTAGE * STAGE_BYTES;  // full[NSTAGE], empty[NSTAGE]
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGE * 8 + 16;
@@ -162,7 +163,7 @@ __device__ __forceinline__ u32x4 philox_staged(uint32_t c0, const PhiloxItem& it
 // Four coupled pairs (one 32-bit word of site bytes per side).  All table lookups are 4-byte shared loads: the phase
 // kernels are bound by shared-memory wavefronts, and with 4-byte entries the hot entries of each table (sigma-sigma pairs,
 // classes without charged neighbours) fall into distinct banks.
-//   move descriptor [key][r], key = fa | fb<<1 | ga<<3 | gb<<4, r = w & 7 (the table of two-site configurations,
+//   move descriptor [r][key], key = fa | fb<<1 | ga<<3 | gb<<4, r = w & 7 (the table of two-site configurations,
 //   PAPER.md:66-74), 8 bytes, 16 copies so that every lane of a half warp reads its own banks (no conflicts at all):
 //   coef = four int8 coefficients;  info = shared-memory address of the class base in the threshold table (low 16 bits) |
 //   xor of the site bytes (a at bits 0,3; b at bits 1,4) << 16.
@@ -177,12 +178,14 @@ __device__ __forceinline__ void pairs4(uint32_t& A4, uint32_t& B4, uint32_t EA4,
   const uint32_t u0 = __byte_perm(FB, GB, 0x5140), u1 = __byte_perm(FB, GB, 0x7362);
   const uint32_t W0 = __byte_perm(t0, u0, 0x5410), W1 = __byte_perm(t0, u0, 0x7632);
   const uint32_t W2 = __byte_perm(t1, u1, 0x5410), W3 = __byte_perm(t1, u1, 0x7632);
-  // key fa | fb<<1 | ga<<3 | gb<<4 (< 28), times 4 in each byte; byte i moved to byte 1 is key * 1024 = its table row
+  // key fa | fb<<1 | ga<<3 | gb<<4 (< 28), times 4 in each byte; a dp4a with the coefficient 32 at byte i gives key * 128,
+  // the offset of the key's 16 private copies in the table [r][key][lane & 15] (address arithmetic on the FMA pipe: the
+  // ALU pipe is the critical resource of this kernel)
   const uint32_t KS = 4u * A4 + 8u * B4;
-  const uint2 q0 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4404) + ((w0 & 7u) << 7));   // s_desc includes (lane & 15) * 8
-  const uint2 q1 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4414) + ((w1 & 7u) << 7));
-  const uint2 q2 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4424) + ((w2 & 7u) << 7));
-  const uint2 q3 = lds_tab64(s_desc + __byte_perm(KS, 0u, 0x4434) + ((w3 & 7u) << 7));
+  const uint2 q0 = lds_tab64((w0 & 7u) * ST_DESC_RSTRIDE + (uint32_t)__dp4a((int)KS, 0x00000020, (int)s_desc));   // s_desc includes (lane & 15) * 8
+  const uint2 q1 = lds_tab64((w1 & 7u) * ST_DESC_RSTRIDE + (uint32_t)__dp4a((int)KS, 0x00002000, (int)s_desc));
+  const uint2 q2 = lds_tab64((w2 & 7u) * ST_DESC_RSTRIDE + (uint32_t)__dp4a((int)KS, 0x00200000, (int)s_desc));
+  const uint2 q3 = lds_tab64((w3 & 7u) * ST_DESC_RSTRIDE + (uint32_t)__dp4a((int)KS, 0x20000000, (int)s_desc));
   const uint32_t f0 = q0.x, i0 = q0.y, f1 = q1.x, i1 = q1.y, f2 = q2.x, i2 = q2.y, f3 = q3.x, i3 = q3.y;
   const uint32_t o0 = (uint32_t)__dp4a((int)W0, (int)f0, (int)(i0 & 0xFFFFu));
   const uint32_t o1 = (uint32_t)__dp4a((int)W1, (int)f1, (int)(i1 & 0xFFFFu));
@@ -216,7 +219,7 @@ __device__ __forceinline__ void st16_left1_tile(uint8_t* row, uint8_t* left, int
 
 // ---------------------------------------------------------------------------------------------------------------
 // The phase kernel.  TYPE: PH_FAR / PH_NEAR_H / PH_NEAR_V; CW: word part of the FAR lane permutation.
-// grid = (blocks, replicas), block = 3 groups of 256 consumer threads + 2 producer warps.
+// grid = (blocks, replicas), block = 3 groups of 256 consumer threads + 3 producer warps.
 // ---------------------------------------------------------------------------------------------------------------
 template <int TYPE, int CW>
 __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_constant__ PhaseArgs A) {
@@ -237,14 +240,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
     uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
     for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_THREADS) {
-      const int key = k >> 7, rr = (k >> 4) & 7;               // keys with bit 2 set do not occur: null entries
+      const int row = k >> 4, rr = row / 28, key = row - 28 * rr;   // keys with bit 2 set do not occur: null entries
       uint2 d = __ldg(&dsrc[key * 8 + rr]);
       d.y += smem0 + C::OFF_THR;                // low 16 bits: shared-memory address of the class base (< 64 KB)
       desc_s[k] = d;
     }
     if (tid == 0) {
       for (int s = 0; s < NST; ++s) {
-        mbar_init(bar0 + 8 * s, ST_NPROD);                              // one arrival per producer warp (+ the bytes of its copies)
+        mbar_init(bar0 + 8 * s, 1);                                     // the producer warp (+ the bytes of its copies)
         mbar_init(bar0 + 8 * (NST + s), ST_TPG / 32);                   // the warps of the consuming group
       }
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -277,69 +280,81 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
   int aF = 0, aT = 0, bF = 0, bT = 0, sgn = 1;   // sums over the new site bytes of the a- and b-sites (sigma_sums)
 
   if (warp >= ST_CONS / 32) {
-    // ============================== producer warp U: region U of every task of the block ================================
-    const int U = warp - ST_CONS / 32;
+    // ============================== producer warp g: both regions of every task of consumer group g =====================
+    const int g = warp - ST_CONS / 32;
     const int kyr = (lane >> 2) - 1, kx = lane & 3;                     // lane = staged row (ky_rel + 1) * 4 + kx
     const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, kyr, kx) : 0;
     const int dY = kyr < 0 ? -1 : kyr > 3 ? 1 : 0;
     const int rowoff = (((kyr & 3) << 2) | kx) << LOGSEG;
     // the edge bytes of a task are loaded one task ahead (their latency hides behind the wait for the ring slot)
-    auto halo_load = [&](int t, uint32_t& hl, uint32_t& hr) {
-      hl = 0u; hr = 0u;
+    auto halo_load = [&](int t, uint32_t (&hl)[2], uint32_t (&hr)[2]) {
+      hl[0] = hl[1] = hr[0] = hr[1] = 0u;
       if (hf && t < ntasks) {
-        const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1), Yr = (Yq + dY) & Wm;
-        if (hf & 1) hl = lat[tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + SEG - 1];
-        if (hf & 2) hr = lat[tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff];
+#pragma unroll
+        for (int U = 0; U < 2; ++U) {
+          const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1), Yr = (Yq + dY) & Wm;
+          if (hf & 1) hl[U] = lat[tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + SEG - 1];
+          if (hf & 2) hr[U] = lat[tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff];
+        }
       }
     };
-    uint32_t hl, hr;
-    halo_load((int)blockIdx.x, hl, hr);
-    for (int t = blockIdx.x, g = 0, k = 0; t < ntasks; t += gridDim.x) {
+    uint32_t hl[2], hr[2];
+    const int tstep = ST_GROUPS * (int)gridDim.x;
+    halo_load((int)blockIdx.x + g * (int)gridDim.x, hl, hr);
+    for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += tstep, ++k) {
       const int s = 2 * g + (k & 1), lap = (k >> 1) & 1;
       const uint32_t full = bar0 + 8 * s;
-      const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1);
+      int Yq[2], sg[2];
+#pragma unroll
+      for (int U = 0; U < 2; ++U) { const int rho = region_of(t, U); Yq[U] = rho >> lognseg; sg[U] = rho & (nseg - 1); }
       mbar_wait(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1), 20000u);
       unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       if (lane == 0) {
-        mbar_expect_tx(full, (uint32_t)C::REGION_BYTES);
-        const uint32_t dst = smem_u32(stg + U * C::REGION_BYTES);
-        if (Yq != 0 && Yq != Wm) {
-          bulk_g2s(dst, lat + tile_off(Yq - 1, sg) + 12 * SEG, C::REGION_BYTES, full);
-        } else if (Yq == 0) {
-          bulk_g2s(dst, lat + tile_off(Wm, sg) + 12 * SEG, 4 * SEG, full);
-          bulk_g2s(dst + 4 * SEG, lat + tile_off(0, sg), (C::ROWS - 4) * SEG, full);
-        } else {
-          bulk_g2s(dst, lat + tile_off(Yq - 1, sg) + 12 * SEG, 20 * SEG, full);
-          bulk_g2s(dst + 20 * SEG, lat + tile_off(0, sg), (C::ROWS - 20) * SEG, full);
+        mbar_expect_tx(full, 2u * (uint32_t)C::REGION_BYTES);
+#pragma unroll
+        for (int U = 0; U < 2; ++U) {
+          const uint32_t dst = smem_u32(stg + U * C::REGION_BYTES);
+          const int Y = Yq[U];
+          if (Y != 0 && Y != Wm) {
+            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * SEG, C::REGION_BYTES, full);
+          } else if (Y == 0) {
+            bulk_g2s(dst, lat + tile_off(Wm, sg[U]) + 12 * SEG, 4 * SEG, full);
+            bulk_g2s(dst + 4 * SEG, lat + tile_off(0, sg[U]), (C::ROWS - 4) * SEG, full);
+          } else {
+            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * SEG, 20 * SEG, full);
+            bulk_g2s(dst + 20 * SEG, lat + tile_off(0, sg[U]), (C::ROWS - 20) * SEG, full);
+          }
         }
       }
-      if (lane >= 30) {
+      if (lane >= 28) {
         // sub-task (U, half): where its items store to, and the coordinates for the Philox counters
-        const int half = lane & 1;
-        SubMeta mt; mt.Y = Yq; mt.C0 = sg << (LOGSEG - 4); mt.pl = 0ull;
+        const int sub = lane - 28, U = sub >> 1, half = sub & 1, Y = Yq[U], seg = sg[U];
+        SubMeta mt; mt.Y = Y; mt.C0 = seg << (LOGSEG - 4); mt.pl = 0ull;
         if (TYPE == PH_FAR) {
-          const int rhoP = paired ? (rho ^ Mrho) : rho;
+          const int UP = paired ? (U ^ 1) : U;
           const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
-          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((ky * 4) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(rhoP >> lognseg, rhoP & (nseg - 1)) + ((kyb * 4) << LOGSEG));
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((ky * 4) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(Yq[UP], sg[UP]) + ((kyb * 4) << LOGSEG));
         } else if (TYPE == PH_NEAR_V) {
-          const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Yq + (ky == 3)) & Wm;
-          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((ky * 4) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(Yb, sg) + ((kyb * 4) << LOGSEG));
+          const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((ky * 4) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(Yb, seg) + ((kyb * 4) << LOGSEG));
         } else {
           const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
-          mt.pa = (unsigned long long)(lat + tile_off(Yq, sg) + ((half * 4 + ka) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(Yq, sg) + ((half * 4 + kb) << LOGSEG));
-          mt.pl = (unsigned long long)(lat + tile_off(Yq, (sg - 1) & (nseg - 1)) + ((half * 4 + ka) << LOGSEG) + SEG - 1);
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((half * 4 + ka) << LOGSEG));
+          mt.pb = (unsigned long long)(lat + tile_off(Y, seg) + ((half * 4 + kb) << LOGSEG));
+          mt.pl = (unsigned long long)(lat + tile_off(Y, (seg - 1) & (nseg - 1)) + ((half * 4 + ka) << LOGSEG) + SEG - 1);
         }
-        *(reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + 2 * U + half) = mt;
+        *(reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + sub) = mt;
       }
-      if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = (uint8_t)hl;
-      if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = (uint8_t)hr;
-      halo_load(t + (int)gridDim.x, hl, hr);
+#pragma unroll
+      for (int U = 0; U < 2; ++U) {
+        if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = (uint8_t)hl[U];
+        if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = (uint8_t)hr[U];
+      }
+      halo_load(t + tstep, hl, hr);
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
-      if (++g == ST_GROUPS) { g = 0; ++k; }
     }
   } else {
     // =========================================== consumer warps ====================================================
