@@ -41,6 +41,7 @@ def lib():
                                        C.POINTER(C.c_uint64), C.POINTER(C.c_int32))
         stp = C.POINTER(OrcState)
         L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]; L.orc_philox4x32_10.restype = None
+        L.orc_philox4x32.argtypes = [u32p, u32p, C.c_int, u32p]; L.orc_philox4x32.restype = None
         L.orc_threshold.argtypes = [C.c_double] * 3 + [C.c_int] * 3 + [C.c_double]; L.orc_threshold.restype = C.c_uint32
         L.orc_recompute.argtypes = [i8p, C.c_int, C.c_int, i64p]; L.orc_recompute.restype = None
         L.orc_pair_table.argtypes = [C.c_int, C.c_int, i8p]; L.orc_pair_table.restype = C.c_int
@@ -71,6 +72,16 @@ def philox4x32_10(ctr, key):
     c = np.asarray(ctr, dtype=np.uint32).copy(); k = np.asarray(key, dtype=np.uint32).copy()
     out = np.zeros(4, dtype=np.uint32)
     lib().orc_philox4x32_10(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(out, C.c_uint32))
+    return out
+
+
+UPDATE_ROUNDS = 7      # Philox rounds of the update stream (ORC_UPDATE_ROUNDS in ic_oracle.h; G5)
+
+
+def philox4x32(ctr, key, rounds):
+    c = np.asarray(ctr, dtype=np.uint32).copy(); k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox4x32(_p(c, C.c_uint32), _p(k, C.c_uint32), int(rounds), _p(out, C.c_uint32))
     return out
 
 

@@ -25,7 +25,8 @@
  * Constraint, eq. (2): sum_i S_i = Q = const.
  *
  * Parity pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
- *   philox4x32_10   known-answer vectors of Salmon et al. (tests/golden/philox_kat.txt)
+ *   philox4x32      10 rounds: known-answer vectors of Salmon et al. (tests/golden/philox_kat.txt); 7 rounds (the
+ *                   update stream): the same vectors with the last three rounds inverted in the test
  *   pair_update     dE closed form (eq. 4,5 with the corrected E_J) == direct
  *                   energy difference from eq. (3) (asserted on EVERY move here,
  *                   and against orc_recompute in the tests); sum S conserved
@@ -53,15 +54,15 @@ static const int S_OF[4] = {0, 0, +1, -1};
 static const int SG_OF[4] = {+1, -1, 0, 0};
 
 /* ------------------------------------------------------------------------- */
-/* U3: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) from its definition. */
+/* U3: Philox4x32-R (Salmon, Moraes, Dror, Shaw, SC'11) from its definition.  */
 /* DESIGN.md reading G5: the paper only says "randomly selected" */
 /* ------------------------------------------------------------------------- */
-void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+void orc_philox4x32(const uint32_t ctr[4], const uint32_t key[2], int rounds, uint32_t out[4]) {
   const uint64_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
   const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
   uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
   uint32_t k0 = key[0], k1 = key[1];
-  for (int round = 0; round < 10; ++round) {
+  for (int round = 0; round < rounds; ++round) {
     uint64_t p0 = M0 * (uint64_t)c0;
     uint64_t p1 = M1 * (uint64_t)c2;
     uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
@@ -73,6 +74,9 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  orc_philox4x32(ctr, key, 10, out);
+}
 
 /* Counter layout:
  *   ctr = (c0, c1, c2, replica | tag<<28),   key = (seed lo, seed hi)          */
@@ -83,7 +87,10 @@ void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2,
                        uint32_t replica, uint32_t tag, uint32_t out[4]) {
   uint32_t ctr[4] = {c0, c1, c2, (replica & 0x0FFFFFFFu) | (tag << 28)};
   uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
-  orc_philox4x32_10(ctr, key, out);
+  /* DESIGN.md G5: the update stream of schedule S1 (one block per four pair updates) is Philox4x32-7, the
+   * seven-round member of the family (Salmon et al. report 7 rounds as the fewest that pass BigCrush, 10 as the
+   * default with a safety margin); every other stream (schedule, stage 1, S0 and the variants) uses 10 rounds. */
+  orc_philox4x32(ctr, key, tag == TAG_UPDATE ? ORC_UPDATE_ROUNDS : 10, out);
 }
 
 /* ------------------------------------------------------------------------- */

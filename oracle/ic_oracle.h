@@ -26,7 +26,11 @@ typedef struct {
   int64_t n_attempt, n_accept, n_null; /* statistics                            */
 } orc_state;
 
+#define ORC_UPDATE_ROUNDS 7 /* Philox rounds of the update stream (G5) */
+void orc_philox4x32(const uint32_t ctr[4], const uint32_t key[2], int rounds, uint32_t out[4]);
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t replica, uint32_t tag, uint32_t out[4]);
+
 uint32_t orc_threshold(double delta, double V, double J, int dn2, int dV, int dJ, double T);
 void orc_recompute(const int8_t* code, int Lx, int Ly, int64_t out6[6]);
 int orc_pair_table(int q, int idx, int8_t out2[2]);
@@ -40,6 +44,7 @@ int64_t orc_schedule_s1(int L, uint64_t seed, uint64_t sweep, int phase, int64_t
 int orc_sweep_s1(orc_state* st, int8_t* code, double T, int64_t nsweeps, int order, int64_t* trace);
 int orc_sweep_s1_mt(orc_state* st, int8_t* code, double T, int64_t nsweeps, int nthreads, int64_t* trace);
 int orc_sweep_s0(orc_state* st, int8_t* code, double T, int64_t nsweeps, int64_t* trace);
+void orc_measure(orc_state* st, int64_t* trace_row);
 
 /* ic_enum.c: exact enumeration */
 int64_t orc_enum_bruteforce(int Lx, int Ly, int64_t* keys /* [cap][6] */, uint64_t* counts, int64_t cap);

@@ -11,7 +11,7 @@
 namespace ic {
 
 // ---------------------------------------------------------------------------------------------------
-// Random numbers: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), counter-based, keyed by the seed.
+// Random numbers: Philox4x32 (Salmon, Moraes, Dror, Shaw, SC'11), counter-based, keyed by the seed.
 // The paper only says pairs and configurations are "randomly selected"; U3.
 // Counter = (c0, c1, c2, replica | tag << 28).
 // ---------------------------------------------------------------------------------------------------
@@ -26,9 +26,10 @@ IC_HD void mulhilo(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
   lo = (uint32_t)p; hi = (uint32_t)(p >> 32);
 }
 
-IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+template <int ROUNDS>
+IC_HD u32x4 philox4x32(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
 #pragma unroll
-  for (int round = 0; round < 10; ++round) {
+  for (int round = 0; round < ROUNDS; ++round) {
     uint32_t h0, l0, h1, l1;
     mulhilo(PHILOX_M0, c0, h0, l0);
     mulhilo(PHILOX_M1, c2, h1, l1);
@@ -36,6 +37,16 @@ IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, ui
     k0 += PHILOX_W0; k1 += PHILOX_W1;
   }
   u32x4 r; r.v[0] = c0; r.v[1] = c1; r.v[2] = c2; r.v[3] = c3; return r;
+}
+// Schedule and stage-1 streams: the default ten rounds.  Update stream (one block per four pair updates, the hot path):
+// Philox4x32-7, the seven-round member of the family that Salmon et al. report as the fewest rounds passing BigCrush
+// (SURVEY 8(d) "RNG ladder", G5).
+constexpr int PHILOX_UPDATE_ROUNDS = 7;
+IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+  return philox4x32<10>(c0, c1, c2, c3, k0, k1);
+}
+IC_HD u32x4 philox_update(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+  return philox4x32<PHILOX_UPDATE_ROUNDS>(c0, c1, c2, c3, k0, k1);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -225,8 +225,8 @@ __global__ void __launch_bounds__(P16_THREADS) k_p16_phase(PhaseArgs A) {
       // random words: block c0 = 4*(X>>2) + kx, c1 = y, word X & 3 with X = x>>2, kx = x&3  (U3)
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        const u32x4 r0 = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + sel), (uint32_t)y, A.c2, c3, A.key0, A.key1);
-        const u32x4 r1 = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + sel + 2), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        const u32x4 r0 = philox_update((uint32_t)(4 * (4 * chunk + j) + sel), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+        const u32x4 r1 = philox_update((uint32_t)(4 * (4 * chunk + j) + sel + 2), (uint32_t)y, A.c2, c3, A.key0, A.key1);
         process4(a_lo.w[j], b_lo.w[j], ea_lo.w[j], eb_lo.w[j], r0.v[0], r0.v[1], r0.v[2], r0.v[3], s_desc, s_thr, acc);
         process4(a_hi.w[j], b_hi.w[j], ea_hi.w[j], eb_hi.w[j], r1.v[0], r1.v[1], r1.v[2], r1.v[3], s_desc, s_thr, acc);
       }
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(P16_THREADS) k_p16_phase(PhaseArgs A) {
         // random words, addressed by the b-site: block c0 = 4*(Xb>>2) + kb, c1 = y, word Xb & 3
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          const u32x4 rr = philox4x32_10((uint32_t)(4 * (4 * chunk + j) + kb), (uint32_t)y, A.c2, c3, A.key0, A.key1);
+          const u32x4 rr = philox_update((uint32_t)(4 * (4 * chunk + j) + kb), (uint32_t)y, A.c2, c3, A.key0, A.key1);
           process4(a.w[j], b.w[j], ea.w[j], eb.w[j], rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, s_thr, acc);
         }
         st16(pb, b);

@@ -69,7 +69,7 @@ __device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL,
     ya = ((p2 + 2 * ((xa + phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
     c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
   }
-  u32x4 rnd = philox4x32_10(c0, (uint32_t)ya, c2, c3, key0, key1);
+  u32x4 rnd = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
   uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
 
   // --- proposal: same pair charge q, configuration r of the paper's list ----------

@@ -137,7 +137,7 @@ __device__ __forceinline__ int halo_flags(int type, int phase, int p2, int kyr, 
   return f;
 }
 
-// Philox4x32-10 with the round keys precomputed on the host (PhaseArgs::rk) and the launch-constant parts of the first two
+// Philox4x32-7 (the update stream, ic_common.cuh) with the round keys precomputed on the host (PhaseArgs::rk) and the launch-constant parts of the first two
 // rounds folded: counter (c0, y, c2, c3), key (k0, k1).  x0 = f0 ^ y and cb = c3 ^ rk[1] are formed once per item / block.
 struct PhiloxItem { uint32_t x0, hi0, lo0; };   // x0 = c0' of round 1 (the same for the four blocks of an item), M0 * x0
 __device__ __forceinline__ u32x4 philox_staged(uint32_t c0, const PhiloxItem& it, uint32_t cb, const PhaseArgs& A) {
@@ -150,7 +150,7 @@ __device__ __forceinline__ u32x4 philox_staged(uint32_t c0, const PhiloxItem& it
   mulhilo(PHILOX_M1, x2, h1, l1);
   uint32_t y0 = h1 ^ A.f2, y1 = l1, y2 = it.hi0 ^ x3 ^ A.rk[3], y3 = it.lo0;
 #pragma unroll
-  for (int round = 2; round < 10; ++round) {
+  for (int round = 2; round < PHILOX_UPDATE_ROUNDS; ++round) {
     uint32_t a, b, c, d;
     mulhilo(PHILOX_M0, y0, a, b);
     mulhilo(PHILOX_M1, y2, c, d);

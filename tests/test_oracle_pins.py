@@ -27,6 +27,27 @@ def test_philox_known_answers(golden_dir):
         assert [int(x) for x in out] == v[6:10]
 
 
+def test_philox_seven_rounds_by_inverting_the_known_answers(golden_dir):
+    """The update stream uses Philox4x32-7 (G5).  Pin: ten rounds = three more rounds on top of seven, and a
+    round is a bijection, so the seven-round output must equal the published ten-round answer with rounds 10, 9, 8
+    undone.  The inverse round is written here from the definition (multiplicative inverses of the odd multipliers
+    modulo 2^32), independently of the oracle's forward code."""
+    M0, M1, W0, W1, MASK = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85, 0xFFFFFFFF
+    I0, I1 = pow(M0, -1, 1 << 32), pow(M1, -1, 1 << 32)
+    rows = [ln.split() for ln in open(os.path.join(golden_dir, "philox_kat.txt")) if ln.strip() and ln[0] != "#"]
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        ctr, key, n = v[0:4], v[4:6], v[6:10]
+        for rnd in (9, 8, 7):                                   # undo round index rnd (key bumped rnd times)
+            k0, k1 = (key[0] + rnd * W0) & MASK, (key[1] + rnd * W1) & MASK
+            c2 = (n[1] * I1) & MASK; c0 = (n[3] * I0) & MASK    # lo words carry M * c mod 2^32
+            c1 = n[0] ^ ((M1 * c2) >> 32) ^ k0; c3 = n[2] ^ ((M0 * c0) >> 32) ^ k1
+            n = [c0, c1, c2, c3]
+        assert [int(x) for x in oracle.philox4x32(ctr, key, 7)] == n
+        assert [int(x) for x in oracle.philox4x32(ctr, key, 10)] == v[6:10]
+    assert oracle.UPDATE_ROUNDS == 7
+
+
 def test_philox_counter_sensitivity():
     base = oracle.philox4x32_10([1, 2, 3, 4], [5, 6])
     for i in range(4):
