@@ -83,26 +83,26 @@ static void build_thresholds(const ic_ctx* c, double T, uint32_t* out) {
   const double qJ = 0.25 * c->J;
   for (int a = -1; a <= 1; ++a)
     for (int v = -16; v <= 16; ++v)
-      for (int j = -16; j <= 16; ++j) out[class_index(2 * a, v, j)] = threshold29(c->delta, c->V, qJ, 2 * a, v, j, T);
+      for (int j = -16; j <= 16; ++j) out[class_index_public(2 * a, v, j)] = threshold29(c->delta, c->V, qJ, 2 * a, v, j, T);
 }
 // Device form of the class table: (8*t29 - 1, packed (dn2, dV, dJ)); w <= 8*t29 - 1  <=>  (w >> 3) < t29.
 static void build_class_table(const ic_ctx* c, double T, uint2* out) {
   uint32_t t29[N_CLASSES];
   build_thresholds(c, T, t29);
+  for (int k = 0; k < THR_STRIDE; ++k) { out[k].x = 0u; out[k].y = 0u; }
   for (int a = -1; a <= 1; ++a)
     for (int v = -16; v <= 16; ++v)
       for (int j = -16; j <= 16; ++j) {
         const int k = class_index(2 * a, v, j);
-        out[k].x = 8u * t29[k] - 1u;
+        out[k].x = 8u * t29[class_index_public(2 * a, v, j)] - 1u;
         out[k].y = (uint32_t)pack_delta(2 * a, v, j);
       }
-  for (int k = N_CLASSES; k < THR_STRIDE; ++k) { out[k].x = 0u; out[k].y = 0u; }
 }
 
 // The table of two-site configurations in the paper's listing order, as move descriptors for the
 // tiled kernels.  Entry [key*8 + r], key = fa | fb<<1 | ga<<3 | gb<<4 in the (f,g) site encoding of LAY_P16:
 //   x = int8 x 4 (cFa, cGa, cFb, cGb): class index = K + cFa*Fa + cGa*Ga + cFb*Fb + cGb*Gb, where the neighbour sums are
-//       sum S = F+G-4, sum sigma = F-G, i.e. cF = 33*dS + dsig, cG = 33*dS - dsig (the -4 cancels: dS_a + dS_b = 0);
+//       sum S = F+G-4, sum sigma = F-G, i.e. cF = CLS_SB*dS + dsig, cG = CLS_SB*dS - dsig (the -4 cancels: dS_a + dS_b = 0);
 //   y = 8*K | (xor of the site bytes: a at bits 0,3, b at bits 1,4) << 16 | (dM & 15 | (dD & 15) << 4) << 24,
 //       K = class_index(E_Delta, adj*dS_a*dS_b, adj*dsig_a*dsig_b)  (eq. 4 for adj = 0, eq. 5 for adj = 1),
 //       dM = dsig_a + dsig_b, dD = dsig_a - dsig_b.
@@ -127,7 +127,7 @@ static void build_descriptors(int adj, uint2* out) {
           const int dSa = S_of(na) - S_of(ca), dSb = S_of(nb) - S_of(cb), dGa = sg_of(na) - sg_of(ca), dGb = sg_of(nb) - sg_of(cb);
           const int e_d = S_of(na) * S_of(na) + S_of(nb) * S_of(nb) - S_of(ca) * S_of(ca) - S_of(cb) * S_of(cb);
           const int K = class_index(e_d, adj * dSa * dSb, adj * dGa * dGb);
-          const int cf[4] = {33 * dSa + dGa, 33 * dSa - dGa, 33 * dSb + dGb, 33 * dSb - dGb};
+          const int cf[4] = {CLS_SB * dSa + dGa, CLS_SB * dSa - dGa, CLS_SB * dSb + dGb, CLS_SB * dSb - dGb};
           d.x = 0u;
           for (int k = 0; k < 4; ++k) d.x |= ((uint32_t)(cf[k] & 0xFF)) << (8 * k);
           const int xa = ea ^ e_of_code(na), xb = eb ^ e_of_code(nb);
@@ -150,10 +150,10 @@ static void build_descriptors32(uint2* out) {
       uint2 q; q.x = 0u; q.y = 4u * (uint32_t)class_index(0, 0, 0);
       if (e < DESC_ENTRIES) {
         const uint2 d = d8[e];
-        // the kernel feeds (4F, 8G) per site: halve the G coefficients (33 dS - dsig is even)
+        // the kernel feeds (4F, 8G) per site: halve the G coefficients (CLS_SB dS - dsig is even: CLS_SB is odd)
         const int cFa = (int8_t)(d.x & 0xFF), cGa = (int8_t)((d.x >> 8) & 0xFF), cFb = (int8_t)((d.x >> 16) & 0xFF), cGb = (int8_t)((d.x >> 24) & 0xFF);
         q.x = (uint32_t)(cFa & 0xFF) | ((uint32_t)((cGa / 2) & 0xFF) << 8) | ((uint32_t)(cFb & 0xFF) << 16) | ((uint32_t)((cGb / 2) & 0xFF) << 24);
-        q.y = ((d.y & 0x7FFFu) >> 1) | (((d.y >> 16) & 0xFFu) << 16);
+        q.y = ((d.y & 0xFFFFu) >> 1) | (((d.y >> 16) & 0xFFu) << 16);
       }
       out[adj * ST_DESC_ENTRIES + e] = q;
     }

@@ -111,12 +111,17 @@ struct Sites {
 };
 
 // Acceptance class of a move (E_Delta, E_V, E_J): dn2 in {-2,0,2}, dV, dJ in [-16,16].
-constexpr int N_CLASSES = 3 * 33 * 33;   // 3267
-constexpr int THR_STRIDE = 3328;         // table entries per replica (multiple of 64)
+constexpr int N_CLASSES = 3 * 33 * 33;   // 3267 (the public, dense order of ic_thresholds)
+// Device order of the class tables: index = (dn2/2+1)*CLS_SA + (dV+16)*CLS_SB + (dJ+16).  The strides decide which
+// shared-memory bank a class falls into; with the dense strides (33, 33*33) the frequent classes collide (bank = dn2/2 + dV
+// + dJ mod 32); 35 spreads them (measured on equilibrated lattices: 2.25 -> 1.53 wavefronts per 32-lane lookup).
+constexpr int CLS_SB = 35, CLS_SA = 33 * CLS_SB;
+constexpr int THR_STRIDE = 3520;         // table entries per replica (>= 3 * CLS_SA, multiple of 64)
 // Device table entry of a class: x = 8*t29 - 1 (the move is accepted iff w <= x, which is (w >> 3) < t29),
 // y = packed (dn2, dV, dJ) = dJ + (dV << 11) + (dn2 << 22) for the per-thread observable accumulator.
 IC_HD int pack_delta(int dn2, int dV, int dJ) { return dJ + dV * 2048 + dn2 * 4194304; }
-IC_HD int class_index(int dn2, int dV, int dJ) { return ((dn2 / 2 + 1) * 33 + (dV + 16)) * 33 + (dJ + 16); }
+IC_HD int class_index(int dn2, int dV, int dJ) { return (dn2 / 2 + 1) * CLS_SA + (dV + 16) * CLS_SB + (dJ + 16); }
+IC_HD int class_index_public(int dn2, int dV, int dJ) { return ((dn2 / 2 + 1) * 33 + (dV + 16)) * 33 + (dJ + 16); }
 
 // Per-replica record in device memory: exact integers, then the fp64 sums of U5.
 struct ReplicaObs {
