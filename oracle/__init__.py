@@ -57,6 +57,13 @@ def lib():
         L.orc_sweep_s1.argtypes = [stp, i8p, C.c_double, C.c_int64, C.c_int, i64p]; L.orc_sweep_s1.restype = C.c_int
         L.orc_sweep_s1_mt.argtypes = [stp, i8p, C.c_double, C.c_int64, C.c_int, i64p]; L.orc_sweep_s1_mt.restype = C.c_int
         L.orc_sweep_s0.argtypes = [stp, i8p, C.c_double, C.c_int64, i64p]; L.orc_sweep_s0.restype = C.c_int
+        u8p, dblp = C.POINTER(C.c_uint8), C.POINTER(C.c_double)
+        L.orc_sweep_nn.argtypes = [stp, i8p, C.c_double, C.c_int64, i64p]; L.orc_sweep_nn.restype = C.c_int
+        L.orc_sweep_mu.argtypes = [stp, i8p, C.c_double, C.c_int64, dblp, C.c_double, C.c_int64, i64p]; L.orc_sweep_mu.restype = C.c_int
+        L.orc_build_map_paper.argtypes = [C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_int64, i64p, i64p]; L.orc_build_map_paper.restype = C.c_int64
+        L.orc_build_map_luby.argtypes = [C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_int64, i64p, i64p, u8p]; L.orc_build_map_luby.restype = C.c_int64
+        L.orc_sweep_maps.argtypes = [stp, i8p, C.c_double, C.c_int64, C.c_int, C.c_int64, i64p, i64p]; L.orc_sweep_maps.restype = C.c_int
+        L.orc_largest_cluster.argtypes = [i8p, C.c_int, C.c_int, C.c_int, i64p]; L.orc_largest_cluster.restype = C.c_int
         L.orc_enum_bruteforce.argtypes = [C.c_int, C.c_int, i64p, u64p, C.c_int64]; L.orc_enum_bruteforce.restype = C.c_int64
         L.orc_enum_rows.argtypes = [C.c_int, C.c_int, C.c_int, i64p, u64p, u64p, u64p, C.c_int64]
         L.orc_enum_rows.restype = C.c_int64
@@ -129,6 +136,31 @@ def schedule_s1(L, seed, sweep, phase):
     return ia[:m], ib[:m], c0[:m], c1[:m], wd[:m]
 
 
+def build_map_paper(Lx, Ly, seed, map_index, npairs):
+    """The paper's sequential map builder: arrays (ia, ib) of the pairs placed."""
+    ia = np.zeros(int(npairs), dtype=np.int64); ib = np.zeros(int(npairs), dtype=np.int64)
+    n = lib().orc_build_map_paper(int(Lx), int(Ly), int(seed), int(map_index), int(npairs), _p(ia, C.c_int64), _p(ib, C.c_int64))
+    return ia[:n], ib[:n]
+
+
+def build_map_luby(Lx, Ly, seed, map_index, K):
+    """K random candidate pairs and which of them survive the one-round conflict resolution: (ia, ib, alive)."""
+    ia = np.zeros(int(K), dtype=np.int64); ib = np.zeros(int(K), dtype=np.int64); alive = np.zeros(int(K), dtype=np.uint8)
+    lib().orc_build_map_luby(int(Lx), int(Ly), int(seed), int(map_index), int(K), _p(ia, C.c_int64), _p(ib, C.c_int64), _p(alive, C.c_uint8))
+    return ia, ib, alive.astype(bool)
+
+
+def largest_cluster(code, which=0):
+    """(size of the largest connected cluster of charged sites, number of clusters); which: 0 any charge, 1 S=+1, 2 S=-1."""
+    code = np.ascontiguousarray(code, dtype=np.int8)
+    Ly, Lx = code.shape
+    out = np.zeros(2, dtype=np.int64)
+    rc = lib().orc_largest_cluster(_p(code, C.c_int8), int(Lx), int(Ly), int(which), _p(out, C.c_int64))
+    if rc != 0:
+        raise MemoryError("orc_largest_cluster")
+    return int(out[0]), int(out[1])
+
+
 class Lattice:
     """One lattice copy driven by the oracle."""
 
@@ -175,6 +207,35 @@ class Lattice:
         if rc != 0:
             raise ValueError(f"orc_sweep_s0 failed with {rc}")
         return tr
+
+    def sweep_nn(self, T, nsweeps, trace=False):
+        """Nearest-neighbour-only coupled pairs: the paper's first, rejected version."""
+        tr = np.zeros((int(nsweeps), 6), dtype=np.int64) if trace else None
+        rc = lib().orc_sweep_nn(C.byref(self.st), _p(self.code, C.c_int8), float(T), int(nsweeps), _p(tr, C.c_int64) if trace else None)
+        if rc != 0:
+            raise ValueError(f"orc_sweep_nn failed with {rc}")
+        return tr
+
+    def sweep_mu(self, T, nsweeps, mu, kappa, q_target, trace=False):
+        """Penalty / chemical-potential single-site Metropolis.  Returns (trace, mu after the run)."""
+        tr = np.zeros((int(nsweeps), 6), dtype=np.int64) if trace else None
+        m = C.c_double(float(mu))
+        rc = lib().orc_sweep_mu(C.byref(self.st), _p(self.code, C.c_int8), float(T), int(nsweeps), C.byref(m), float(kappa),
+                                int(q_target), _p(tr, C.c_int64) if trace else None)
+        if rc != 0:
+            raise ValueError(f"orc_sweep_mu failed with {rc}")
+        return tr, m.value
+
+    def sweep_maps(self, T, nmaps, mode, K, trace=False):
+        """Sweeps made of maps: mode 0 the paper's sequential builder, 1 one-round conflict resolution.
+        Returns (trace, number of attempted pair updates)."""
+        tr = np.zeros((int(nmaps), 6), dtype=np.int64) if trace else None
+        att = C.c_int64(0)
+        rc = lib().orc_sweep_maps(C.byref(self.st), _p(self.code, C.c_int8), float(T), int(nmaps), int(mode), int(K),
+                                  _p(tr, C.c_int64) if trace else None, C.byref(att))
+        if rc != 0:
+            raise ValueError(f"orc_sweep_maps failed with {rc}")
+        return tr, att.value
 
     def observables(self, T):
         """U5: C = (<E^2>-<E>^2)/(N T^2) (k=1); chi = (<M^2>-<M>^2)/(N T) (reading G9)."""

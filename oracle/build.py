@@ -7,7 +7,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["ic_oracle.c", "ic_enum.c"]
+SOURCES = ["ic_oracle.c", "ic_variants.c", "ic_enum.c"]
 LIB = os.path.join(HERE, "libic_oracle.so")
 
 

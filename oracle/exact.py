@@ -51,6 +51,19 @@ def averages(dos, Q, delta, V, J, T):
     return out
 
 
+def averages_grand(dos, mu, delta, V, J, T):
+    """Grand-canonical averages over ALL charge sectors with weights exp(-(E - mu Q)/T): what single-site Metropolis
+    with the extra term -mu sum S samples at fixed mu.  Returns <E>, <E^2>, <Q>, <Q^2>."""
+    keys, counts, _, _ = dos
+    E = (delta * keys[:, 1].astype(float) + V * keys[:, 2].astype(float)) + (0.25 * J) * keys[:, 3].astype(float)
+    Qs = keys[:, 0].astype(float)
+    H = E - mu * Qs
+    w = counts.astype(float) * np.exp(-(H - H.min()) / T)
+    Z = float(w.sum())
+    return dict(E=float((w * E).sum()) / Z, E2=float((w * E * E).sum()) / Z, Q=float((w * Qs).sum()) / Z,
+                Q2=float((w * Qs * Qs).sum()) / Z)
+
+
 def dos_from_bruteforce(keys6, counts):
     """Collapse brute-force keys (n2,bV,bJ,M,Ms,Q) to the (Q,n2,bV,bJ) form used by `averages`."""
     acc = {}

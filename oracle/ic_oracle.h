@@ -46,6 +46,15 @@ int orc_sweep_s1_mt(orc_state* st, int8_t* code, double T, int64_t nsweeps, int 
 int orc_sweep_s0(orc_state* st, int8_t* code, double T, int64_t nsweeps, int64_t* trace);
 void orc_measure(orc_state* st, int64_t* trace_row);
 
+/* ic_variants.c: what the paper describes around the main algorithm (negative controls, maps, drop observable) */
+int orc_sweep_nn(orc_state* st, int8_t* code, double T, int64_t nsweeps, int64_t* trace);
+int orc_sweep_mu(orc_state* st, int8_t* code, double T, int64_t nsweeps, double* mu, double kappa, int64_t q_target,
+                 int64_t* trace);
+int64_t orc_build_map_paper(int Lx, int Ly, uint64_t seed, uint64_t map_index, int64_t npairs, int64_t* ia, int64_t* ib);
+int64_t orc_build_map_luby(int Lx, int Ly, uint64_t seed, uint64_t map_index, int64_t K, int64_t* ia, int64_t* ib, uint8_t* alive);
+int orc_sweep_maps(orc_state* st, int8_t* code, double T, int64_t nmaps, int mode, int64_t K, int64_t* trace, int64_t* attempted);
+int orc_largest_cluster(const int8_t* code, int Lx, int Ly, int which, int64_t out2[2]);
+
 /* ic_enum.c: exact enumeration */
 int64_t orc_enum_bruteforce(int Lx, int Ly, int64_t* keys /* [cap][6] */, uint64_t* counts, int64_t cap);
 int64_t orc_enum_rows(int Lx, int Ly, int nthreads, int64_t* keys /* [cap][4] */, uint64_t* counts,

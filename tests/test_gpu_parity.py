@@ -236,9 +236,10 @@ def test_config_c1_full_length(pkg):
 
 
 def test_config_c2_batched_replicas(pkg):
-    """BASELINE config 2: L=64, 64 temperatures as 64 replicas in one launch (reduced sweep count on the oracle side)."""
+    """BASELINE config 2 at full length: L=64, 64 temperatures as 64 replicas in one launch, 10^4 sweeps,
+    both state widths, every replica against the oracle."""
     c = ic_inputs.CONFIGS["C2"]
-    L, Ts, nsw = c["L"], c["T"], 400
+    L, Ts, nsw = c["L"], c["T"], c["sweeps"]
     codes = [ic_inputs.random_state(L, c["nplus"], 0, c["seed"], r) for r in range(len(Ts))]
     for bits in (8, 2):
         sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=len(Ts), bits_per_site=bits)
@@ -252,9 +253,10 @@ def test_config_c2_batched_replicas(pkg):
 
 
 def test_config_c3_packed_l1024(pkg):
-    """BASELINE config 3: L=1024, neutral with both charge signs at density 0.3, 2-bit packed state."""
+    """BASELINE config 3 at full length: L=1024, neutral with both charge signs at density 0.3, 2-bit packed
+    state, 10^3 sweeps."""
     c = ic_inputs.CONFIGS["C3"]
-    L, nsw = c["L"], 24
+    L, nsw = c["L"], c["sweeps"]
     code = ic_inputs.random_state(L, c["nplus"], c["nminus"], c["seed"])
     sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=2); sim.set_state(0, code)
     lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
@@ -263,43 +265,85 @@ def test_config_c3_packed_l1024(pkg):
     sim.close()
 
 
-def test_config_c4_trace_l4096(pkg):
-    """BASELINE config 4 (2 of its 16 replicas on the oracle side): per-sweep integers via ic_sweep_trace."""
+@pytest.mark.parametrize("bits", [8, 2])
+def test_config_c4_trace_l4096(pkg, bits):
+    """BASELINE config 4 in the launch shape bench.py --config C4 times (L=4096, all 16 replicas in one launch: grid
+    (sm_count / 16, 16) for the staged kernels): per-sweep integers via ic_sweep_trace for the first 20 sweeps against the
+    oracle, replica by replica, then on to 500 sweeps with eq. (2) and incremental == recomputed integers on every replica
+    (SURVEY 8(d))."""
     c = ic_inputs.CONFIGS["C4"]
-    L, nsw = c["L"], 4
-    Ts = [c["T"][0], c["T"][15]]
-    codes = [ic_inputs.random_state(L, c["nplus"], 0, c["seed"], r) for r in range(2)]
-    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=2, bits_per_site=8)
-    for r in range(2):
-        sim.set_state(r, codes[r])
+    L, Ts, reps, nsw = c["L"], c["T"], len(c["T"]), 20
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], replicas=reps, bits_per_site=bits)
+    codes = [sim.state(r).copy() for r in range(reps)]                   # stage-1 states of ic_create
+    for r in (0, reps - 1):
+        assert np.array_equal(codes[r], oracle.init_state(L, L, c["nplus"], 0, c["seed"], r))
     tr = sim.sweep_trace(Ts, nsw).cpu().numpy()
-    lats = [oracle.Lattice(codes[r], c["delta"], c["V"], c["J"], c["seed"], replica=r) for r in range(2)]
-    for r in range(2):
-        t = lats[r].sweep_s1(Ts[r], nsw, trace=True, threads=NCPU)
-        assert np.array_equal(tr[:, r, :], t)
-    check_against_oracle(sim, lats, Ts)
+    per = max(1, NCPU // 4)
+
+    def go(r):
+        lat = oracle.Lattice(codes[r], c["delta"], c["V"], c["J"], c["seed"], replica=r)
+        t = lat.sweep_s1(Ts[r], nsw, trace=True, threads=per)
+        return lat, t
+
+    with ThreadPoolExecutor(max_workers=4) as ex:
+        res = list(ex.map(go, range(reps)))
+    for r in range(reps):
+        assert np.array_equal(tr[:, r, :], res[r][1]), f"per-sweep integers differ, replica {r}"
+    check_against_oracle(sim, [lt for lt, _ in res], Ts)
+    tr2 = sim.sweep_trace(Ts, c["sweeps"] - nsw).cpu().numpy()
+    assert (tr2[:, :, 5] == sim.Q).all()                                  # eq. (2) after every sweep, every replica
+    obs = sim.observables()
+    for r in range(reps):
+        assert obs[r]["nmeas"] == c["sweeps"]
+        assert list(sim.debug_recompute(r)) == [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+        assert list(tr2[-1, r, :]) == [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     sim.close()
 
 
-def test_config_c5_full_size_sampled(pkg):
-    """BASELINE config 5 at its full size (L=16384, the launch configuration bench.py times): two sweeps (one FAR, one
-    NEAR) against the multi-threaded oracle, whole lattice compared; then invariants after more sweeps."""
+@pytest.mark.parametrize("bits", [8, 2])
+def test_config_c5_full_size_sampled(pkg, bits):
+    """BASELINE config 5 at its full size (L=16384, the launch configuration bench.py times): the first 5 sweeps against
+    the multi-threaded oracle, whole lattice compared; then eq. (2) and incremental == recomputed integers after all 100
+    sweeps; also at 2 bits per site."""
     c = ic_inputs.CONFIGS["C5"]
     L = c["L"]
-    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=8)
+    sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=bits)
     code = sim.state(0).copy()
     assert int(S_OF[code].sum()) == sim.Q == c["nplus"]
     lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
-    sim.sweep(c["T"], 2); lat.sweep_s1(c["T"][0], 2, threads=NCPU)
+    sim.sweep(c["T"], 5); lat.sweep_s1(c["T"][0], 5, threads=NCPU)
     got = sim.state(0)
     assert np.array_equal(got, lat.code)
     o = sim.observables()[0]; ref = lat.observables(c["T"][0])
     for k in ("n2", "bV", "bJ", "M", "Ms", "Q", "sumE", "sumE2", "sumM2", "sumMs2"):
         assert o[k] == ref[k], (k, o[k], ref[k])
-    sim.sweep(c["T"], 6)
+    sim.sweep(c["T"], c["sweeps"] - 5)
     assert int(S_OF[sim.state(0)].sum()) == sim.Q
     o = sim.observables()[0]
+    assert o["nmeas"] == c["sweeps"]
     assert list(sim.debug_recompute(0)) == [o[k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    sim.close()
+
+
+def test_staged_kernels_one_block_per_replica(pkg):
+    """More replicas than SMs: the staged kernels run with gridDim.x = 1 (one persistent block per replica walks the whole
+    lattice).  L=2048, 160 replicas; three replicas against the oracle, every replica against eq. (2) and the recount."""
+    import torch
+    L, reps, seed = 2048, torch.cuda.get_device_properties(0).multi_processor_count + 12, 31
+    Ts = [0.3 + 0.01 * r for r in range(reps)]
+    sim = pkg.Sim(L, 0.1, 0.5, 1.0, 1.0, seed=seed, replicas=reps); sim.set_variant(3)
+    picks = [0, reps // 2, reps - 1]
+    codes = {r: sim.state(r).copy() for r in picks}
+    sim.sweep(Ts, 4)
+    obs = sim.observables()
+    for r in picks:
+        lat = oracle.Lattice(codes[r], 0.5, 1.0, 1.0, seed, replica=r)
+        lat.sweep_s1(Ts[r], 4, threads=NCPU)
+        assert np.array_equal(sim.state(r), lat.code), r
+        assert [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")] == list(lat.ints())
+    for r in range(0, reps, 7):
+        assert obs[r]["Q"] == sim.Q
+        assert list(sim.debug_recompute(r)) == [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     sim.close()
 
 

@@ -127,3 +127,31 @@ def test_ising_limit_orders_antiferromagnetically():
     hot.sweep_s1(5.0, 100)
     tr = hot.sweep_s1(5.0, 200, trace=True)
     assert np.abs(tr[:, 4]).mean() < 0.3 * L * L                                      # melts above T_c
+
+
+@pytest.mark.parametrize("L", [64, 256, 1024])
+def test_random_word_address_is_the_stated_function_of_the_slot_site(L):
+    """DESIGN.md U3 "Random-word address": the pair whose slot site is (x, y) -- its a-site, or its b-site for horizontal
+    dominoes -- uses word (x >> 2) & 3 of the Philox block with counter c0 = 4 (x >> 4) + (x & 3), c1 = y.  Stated here
+    as a plain function of (x, y) and checked for every pair of FAR, NEAR-H and NEAR-V sweeps at sizes where x >> 4 > 0
+    (the sampling pins run at L = 4, where it is always 0); addresses are unique within a phase."""
+    seen_types = set()
+    sweep = 0
+    while len(seen_types) < 3 and sweep < 64:
+        par = oracle.schedule_params(L, 31, sweep)
+        kind = "far" if par[0] == 0 else ("near_h" if par[1] == 0 else "near_v")
+        if kind in seen_types:
+            sweep += 1
+            continue
+        seen_types.add(kind)
+        for phase in (0, 1):
+            ia, ib, c0, c1, wd = oracle.schedule_s1(L, 31, sweep, phase)
+            assert len(ia) == L * L // 4
+            slot = ib if kind == "near_h" else ia
+            x, y = slot % L, slot // L
+            assert (c0 == 4 * (x >> 4) + (x & 3)).all() and (c1 == y).all() and (wd == ((x >> 2) & 3)).all()
+            assert (c0 >= 4).any() and c0.max() < L // 4                  # blocks beyond the first 16 columns occur
+            key = (c1.astype(np.int64) * (L // 4) + c0.astype(np.int64)) * 4 + wd.astype(np.int64)
+            assert len(np.unique(key)) == len(key)
+        sweep += 1
+    assert seen_types == {"far", "near_h", "near_v"}
