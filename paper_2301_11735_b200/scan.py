@@ -1,8 +1,9 @@
 """Temperature scan: heat capacity C(T) and magnetic susceptibilities chi(T) with error bars.
 
 The step after the hot path and the paper's main result (PAPER.md:49-53, 161, 188 / Fig. 6): all temperatures run as
-replicas of one `Sim` (one launch per sweep phase, or one launch per call for L <= 64), the per-sweep integers
-(n2, bV, bJ, M, Ms) come back through `ic_sweep_trace`, and this module only does the statistics on the host:
+replicas of one `Sim` (one launch per sweep phase, or one launch per call for L <= 64); E, E^2, M, M^2, ... are accumulated
+per sweep by the library (`ic_observables`), read and reset once per block, and this module only does the statistics over
+blocks on the host:
 
     E = Delta*n2 + V*bV + (J/4)*bJ                                   (eq. 3)
     C = (<E^2> - <E>^2) / (N T^2)                                    (k_B = 1)
@@ -30,10 +31,10 @@ def _jackknife(blocks, f):
     return full, err
 
 
-def temperature_scan(L, n, delta, V, J, Ts, equil, sweeps, seed=1, bins=32, bits_per_site=8, chunk=50000, init_charges=None):
+def temperature_scan(L, n, delta, V, J, Ts, equil, sweeps, seed=1, bins=32, bits_per_site=8, init_charges=None):
     """Runs len(Ts) replicas at temperatures Ts: `equil` sweeps discarded, `sweeps` measured.  Returns a dict of numpy
-    arrays over the temperatures: T, E, E_err, C, C_err, chi_u, chi_u_err, chi_s, chi_s_err, absM, absMs, n2 and the
-    exact integer charge Q (eq. 2 is checked on every measured sweep)."""
+    arrays over the temperatures: T, E, E_err, C, C_err, chi_u, chi_u_err, chi_s, chi_s_err, absM, absMs and the
+    exact integer charge Q (eq. 2 is checked after every block)."""
     Ts = [float(t) for t in Ts]
     reps = len(Ts)
     if sweeps < bins or bins < 2:
@@ -49,31 +50,26 @@ def temperature_scan(L, n, delta, V, J, Ts, equil, sweeps, seed=1, bins=32, bits
         N = float(L) * float(L)
         per_bin = sweeps // bins
         used = per_bin * bins
-        # per-block means of (E, E^2, M, M^2, |M|, Ms, Ms^2, |Ms|, n2), accumulated chunk by chunk
-        acc = np.zeros((reps, bins, 9))
-        done = 0
-        while done < used:
-            m = int(min(chunk, used - done))
-            tr = sim.sweep_trace(Ts, m).cpu().numpy()                 # [m, reps, 6] = n2, bV, bJ, M, Ms, Q
-            if not (tr[:, :, 5] == sim.Q).all():
-                raise RuntimeError("charge not conserved (eq. 2)")
-            n2 = tr[:, :, 0].astype(np.float64); bV = tr[:, :, 1].astype(np.float64); bJ = tr[:, :, 2].astype(np.float64)
-            E = (delta * n2 + V * bV) + (0.25 * J) * bJ
-            M = tr[:, :, 3].astype(np.float64); Ms = tr[:, :, 4].astype(np.float64)
-            q = np.stack([E, E * E, M, M * M, np.abs(M), Ms, Ms * Ms, np.abs(Ms), n2], axis=2)   # [m, reps, 9]
-            idx = (done + np.arange(m)) // per_bin
-            for b in np.unique(idx):
-                acc[:, b, :] += q[idx == b].sum(axis=0)
-            done += m
-        acc /= per_bin
-        out = {k: np.zeros(reps) for k in ("E", "E_err", "C", "C_err", "chi_u", "chi_u_err", "chi_s", "chi_s_err", "absM", "absMs", "n2")}
+        # per-block means of (E, E^2, M, M^2, |M|, Ms, Ms^2, |Ms|): the library's own fp64 accumulators (A9), read and
+        # reset once per block -- the host does statistics over blocks only
+        acc = np.zeros((reps, bins, 8))
+        keys = ("sumE", "sumE2", "sumM", "sumM2", "sumAbsM", "sumMs", "sumMs2", "sumAbsMs")
+        for b in range(bins):
+            sim.reset_observables()
+            sim.sweep(Ts, per_bin)
+            obs = sim.observables()
+            for r in range(reps):
+                if obs[r]["Q"] != sim.Q or obs[r]["nmeas"] != per_bin:
+                    raise RuntimeError("charge not conserved (eq. 2) or sweeps lost")
+                acc[r, b, :] = [obs[r][k] / per_bin for k in keys]
+        out = {k: np.zeros(reps) for k in ("E", "E_err", "C", "C_err", "chi_u", "chi_u_err", "chi_s", "chi_s_err", "absM", "absMs")}
         for r, T in enumerate(Ts):
             blk = acc[r]
             out["E"][r], out["E_err"][r] = _jackknife(blk, lambda v: v[0])
             out["C"][r], out["C_err"][r] = _jackknife(blk, lambda v: (v[1] - v[0] * v[0]) / (N * T * T))
             out["chi_u"][r], out["chi_u_err"][r] = _jackknife(blk, lambda v: (v[3] - v[2] * v[2]) / (N * T))
             out["chi_s"][r], out["chi_s_err"][r] = _jackknife(blk, lambda v: (v[6] - v[5] * v[5]) / (N * T))
-            out["absM"][r] = blk[:, 4].mean(); out["absMs"][r] = blk[:, 7].mean(); out["n2"][r] = blk[:, 8].mean()
+            out["absM"][r] = blk[:, 4].mean(); out["absMs"][r] = blk[:, 7].mean()
         out["T"] = np.array(Ts); out["Q"] = sim.Q; out["sweeps"] = used; out["bins"] = bins
         return out
     finally:

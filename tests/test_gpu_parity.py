@@ -18,6 +18,7 @@ pytestmark = pytest.mark.gpu
 
 NCPU = os.cpu_count() or 1
 S_OF = np.array([0, 0, 1, -1])
+_ORACLE_RUNS = {}     # oracle results shared by the two state widths of a config (identical inputs, identical expected lattices)
 
 
 @pytest.fixture(scope="module")
@@ -285,8 +286,11 @@ def test_config_c4_trace_l4096(pkg, bits):
         t = lat.sweep_s1(Ts[r], nsw, trace=True, threads=per)
         return lat, t
 
-    with ThreadPoolExecutor(max_workers=4) as ex:
-        res = list(ex.map(go, range(reps)))
+    if "C4" not in _ORACLE_RUNS:
+        with ThreadPoolExecutor(max_workers=4) as ex:
+            _ORACLE_RUNS["C4"] = (codes, list(ex.map(go, range(reps))))
+    codes0, res = _ORACLE_RUNS["C4"]
+    assert all(np.array_equal(a, b) for a, b in zip(codes, codes0))       # the oracle run started from these very states
     for r in range(reps):
         assert np.array_equal(tr[:, r, :], res[r][1]), f"per-sweep integers differ, replica {r}"
     check_against_oracle(sim, [lt for lt, _ in res], Ts)
@@ -310,8 +314,13 @@ def test_config_c5_full_size_sampled(pkg, bits):
     sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=bits)
     code = sim.state(0).copy()
     assert int(S_OF[code].sum()) == sim.Q == c["nplus"]
-    lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
-    sim.sweep(c["T"], 5); lat.sweep_s1(c["T"][0], 5, threads=NCPU)
+    sim.sweep(c["T"], 5)
+    if "C5" not in _ORACLE_RUNS:
+        lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
+        lat.sweep_s1(c["T"][0], 5, threads=NCPU)
+        _ORACLE_RUNS["C5"] = (code, lat)
+    code0, lat = _ORACLE_RUNS["C5"]
+    assert np.array_equal(code, code0)
     got = sim.state(0)
     assert np.array_equal(got, lat.code)
     o = sim.observables()[0]; ref = lat.observables(c["T"][0])
