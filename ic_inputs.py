@@ -22,6 +22,11 @@ CONFIGS = {
                sweeps=500, equil=0, bits=8, seed=4),
     "C5": dict(L=16384, n=0.05, delta=0.2, V=1.0, J=1.0, T=[1.0], nplus=13421773, nminus=0,
                sweeps=100, equil=0, bits=8, seed=5),
+    # second workload of the paper (Fig. 7): formation of a charge "drop" on a 64 x 64 lattice with a
+    # strong magnetic exchange J >> V; the paper gives no parameters (figure only), these are ours: a quench from a random
+    # state at four temperatures
+    "C6": dict(L=64, n=0.1, delta=0.0, V=0.1, J=4.0, T=[0.2, 0.4, 0.8, 1.6], nplus=410, nminus=0,
+               sweeps=4000, equil=0, bits=8, seed=6),
 }
 
 

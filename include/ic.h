@@ -118,6 +118,32 @@ int ic_schedule(ic_ctx* ctx, uint64_t sweep, int32_t* out4);
 int64_t ic_sweep_count(const ic_ctx* ctx);        /* global sweep counter; -1 if ctx is NULL           */
 int64_t ic_charge(const ic_ctx* ctx);             /* Q = llround(n*N); 0 if ctx is NULL                */
 
+/* ---- maps: the paper's own parallel schedule (sec. 3.2) as an alternative to ic_sweep ----------------
+ * A "map" is a randomly generated list of coupled pairs that do not interact: no site of one pair equals or neighbours a
+ * site of another (Fig. 1), so all pairs of a map are updated in parallel, one thread each, the
+ * same map for every lattice copy.  The paper builds maps of N/10 pairs sequentially on the CPU
+ * and ships them over PCIe; here every map is built on the device in one round: K candidate pairs of
+ * two distinct uniformly random sites (counter-based stream keyed by the seed and the map index); candidate k is kept iff
+ * no candidate of lower index has a site inside its covering (its two sites and their nearest neighbours).
+ * ic_sweep_maps runs nmaps maps; after each map ("step" of PAPER.md:167) E, E^2, ... are accumulated as after a sweep and,
+ * if d_trace is not NULL, (n2,bV,bJ,M,Ms,Q) are written to d_trace[m][r][6] (DEVICE).  The map index is the context's
+ * sweep counter, which advances by one per map.  d_scratch: DEVICE memory of ic_maps_scratch_bytes(L, K) bytes, 256-B
+ * aligned, caller-owned, free to reuse after the call's work has finished on the stream.  L <= 32768.
+ * Errors: IC_ERR_SIZE (K < 1, L too large), IC_ERR_PARAM (T, nmaps), IC_ERR_WORKSPACE.                                   */
+size_t ic_maps_scratch_bytes(int L, int64_t K);
+int ic_sweep_maps(ic_ctx* ctx, const double* h_T, int64_t nmaps, int64_t K, void* d_scratch, size_t scratch_bytes,
+                  int64_t* d_trace);
+
+/* ---- the "drop" (Fig. 7: with J >> V the whole charge gathers in one place) --------------------------
+ * ic_largest_cluster: h_out2 = (size of the largest connected cluster of charged sites, number of clusters) of one
+ * replica; 4-neighbour connectivity, periodic; which = 0: sites with S != 0, 1: S = +1, 2: S = -1.  d_scratch: DEVICE
+ * memory of ic_cluster_scratch_bytes(L) bytes, 256-B aligned.  Synchronises the stream.  L <= 32768.
+ * ic_snapshot_ppm: writes the replica's lattice as a binary PPM image (one pixel per site: S=+1 red, S=-1 blue,
+ * sigma=+1 white, sigma=-1 grey) from host memory to `path`; IC_ERR_PARAM if the file cannot be opened.                   */
+size_t ic_cluster_scratch_bytes(int L);
+int ic_largest_cluster(ic_ctx* ctx, int replica, int which, void* d_scratch, size_t scratch_bytes, int64_t* h_out2);
+int ic_snapshot_ppm(ic_ctx* ctx, int replica, const char* path);
+
 /* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
  * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels
  * (8 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default there).

@@ -37,6 +37,11 @@ EXPORTS = {
     "ic_debug_recompute": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "ic_thresholds": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(C.c_uint32)]),
     "ic_schedule": (C.c_int, [C.c_void_p, C.c_uint64, C.POINTER(C.c_int32)]),
+    "ic_maps_scratch_bytes": (C.c_size_t, [C.c_int, C.c_int64]),
+    "ic_sweep_maps": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_int64, C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "ic_cluster_scratch_bytes": (C.c_size_t, [C.c_int]),
+    "ic_largest_cluster": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.POINTER(C.c_int64)]),
+    "ic_snapshot_ppm": (C.c_int, [C.c_void_p, C.c_int, C.c_char_p]),
     "ic_sweep_count": (C.c_int64, [C.c_void_p]),
     "ic_charge": (C.c_int64, [C.c_void_p]),
     "ic_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
@@ -122,6 +127,37 @@ class Sim:
         tr = self.torch.empty((int(nsweeps), self.replicas, 6), dtype=self.torch.int64, device=self.device)
         _check(lib.ic_sweep_trace(self.h, p, int(nsweeps), C.c_void_p(tr.data_ptr())), "ic_sweep_trace")
         return tr
+
+    def _scratch(self, nbytes):
+        """A 256-byte aligned device buffer of at least nbytes (kept and reused)."""
+        if nbytes == 0:
+            raise IcError(IC_ERR_SIZE, "scratch size")
+        buf = getattr(self, "_scratch_buf", None)
+        if buf is None or buf.numel() < nbytes + 256:
+            with self.torch.cuda.device(self.device):
+                self._scratch_buf = buf = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device=self.device)
+        return (buf.data_ptr() + 255) & ~255
+
+    def sweep_maps(self, T, nmaps, K, trace=False):
+        """nmaps device-built maps of K candidate pairs each; returns the per-map trace if asked."""
+        arr, p = self._T(T)
+        nbytes = lib.ic_maps_scratch_bytes(self.L, int(K))
+        ptr = self._scratch(nbytes)
+        tr = self.torch.empty((int(nmaps), self.replicas, 6), dtype=self.torch.int64, device=self.device) if trace else None
+        _check(lib.ic_sweep_maps(self.h, p, int(nmaps), int(K), C.c_void_p(ptr), nbytes,
+                                 C.c_void_p(tr.data_ptr()) if trace else None), "ic_sweep_maps")
+        return tr
+
+    def largest_cluster(self, replica=0, which=0):
+        """(size of the largest connected cluster of charged sites, number of clusters)."""
+        nbytes = lib.ic_cluster_scratch_bytes(self.L)
+        ptr = self._scratch(nbytes)
+        out = (C.c_int64 * 2)()
+        _check(lib.ic_largest_cluster(self.h, int(replica), int(which), C.c_void_p(ptr), nbytes, out), "ic_largest_cluster")
+        return int(out[0]), int(out[1])
+
+    def snapshot_ppm(self, replica, path):
+        _check(lib.ic_snapshot_ppm(self.h, int(replica), os.fsencode(path)), "ic_snapshot_ppm")
 
     def reset_observables(self):
         _check(lib.ic_reset_observables(self.h), "ic_reset_observables")

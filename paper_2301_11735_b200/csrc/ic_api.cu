@@ -18,6 +18,7 @@
 #include "ic_kernels_p16.cuh"
 #include "ic_kernels_staged.cuh"
 #include "ic_kernels_resident.cuh"
+#include "ic_kernels_extra.cuh"
 
 using namespace ic;
 
@@ -493,14 +494,8 @@ static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
   return IC_OK;
 }
 
-static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_trace) {
-  if (!c || !h_T) return IC_ERR_NULL;
-  if (nsweeps < 0 || c->sweep + (uint64_t)nsweeps >= (1ull << 31)) return IC_ERR_PARAM;
-  for (int r = 0; r < c->replicas; ++r)
-    if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
-  if (nsweeps == 0) return IC_OK;
-
-  // thresholds: rebuilt and uploaded only when a temperature changed
+// thresholds: rebuilt and uploaded only when a temperature changed
+static int ensure_thresholds(ic_ctx* c, const double* h_T) {
   bool changed = !c->have_T;
   for (int r = 0; r < c->replicas && !changed; ++r) changed = (*c->lastT)[r] != h_T[r];
   if (changed) {
@@ -514,6 +509,18 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     IC_CUDA(cudaEventRecord(c->thr_copied, c->stream));
     c->have_T = true;
   }
+
+  return IC_OK;
+}
+
+static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_trace) {
+  if (!c || !h_T) return IC_ERR_NULL;
+  if (nsweeps < 0 || c->sweep + (uint64_t)nsweeps >= (1ull << 31)) return IC_ERR_PARAM;
+  for (int r = 0; r < c->replicas; ++r)
+    if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
+  if (nsweeps == 0) return IC_OK;
+
+  { int rc = ensure_thresholds(c, h_T); if (rc != IC_OK) return rc; }
 
   // small lattices: all the sweeps in one launch, one block per replica, lattice resident in shared memory
   if (c->L <= RES_MAX_L && (c->variant == 0 || c->variant == 4)) {
@@ -613,6 +620,99 @@ extern "C" int ic_debug_recompute(ic_ctx* c, int replica, int64_t* out6) {
   IC_CUDA(cudaMemcpyAsync(h, c->d_scratch8, 64, cudaMemcpyDeviceToHost, c->stream));
   IC_CUDA(cudaStreamSynchronize(c->stream));
   for (int k = 0; k < 6; ++k) out6[k] = h[k];
+  return IC_OK;
+}
+
+
+// ---- maps -----------------------------------------------------------------------------------------
+static bool small_index_ok(const ic_ctx* c) { return c->L <= 32768; }   // site indices as int32
+
+extern "C" size_t ic_maps_scratch_bytes(int L, int64_t K) {
+  if (L < 4 || L > 32768 || (L & (L - 1)) || K < 1 || K > (1LL << 30)) return 0;
+  return align256((size_t)L * L * 4) + align256((size_t)K * 8) + 256;
+}
+
+extern "C" int ic_sweep_maps(ic_ctx* c, const double* h_T, int64_t nmaps, int64_t K, void* d_scratch, size_t scratch_bytes,
+                             int64_t* d_trace) {
+  if (!c || !h_T) return IC_ERR_NULL;
+  if (!small_index_ok(c) || K < 1 || K > (1LL << 30)) return IC_ERR_SIZE;
+  if (nmaps < 0 || c->sweep + (uint64_t)nmaps >= (1ull << 31)) return IC_ERR_PARAM;
+  for (int r = 0; r < c->replicas; ++r)
+    if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
+  if (!d_scratch || scratch_bytes < ic_maps_scratch_bytes(c->L, K) || ((uintptr_t)d_scratch & 255) != 0) return IC_ERR_WORKSPACE;
+  if (nmaps == 0) return IC_OK;
+  { int rc = ensure_thresholds(c, h_T); if (rc != IC_OK) return rc; }
+  MapArgs a;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
+  a.first = (int*)d_scratch; a.ia = (int*)((char*)d_scratch + align256((size_t)c->N * 4)); a.ib = a.ia + K;
+  a.L = c->L; a.logL = c->logL; a.K = (int)K; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
+  const double qJ = 0.25 * c->J;
+  const int nb_reset = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);
+  const unsigned nb_k = (unsigned)((K + 255) / 256);
+  for (int64_t m = 0; m < nmaps; ++m) {
+    a.map_index = (uint32_t)c->sweep;
+    k_map_reset<<<nb_reset, 256, 0, c->stream>>>(a.first, c->N, (int)K);
+    k_map_candidates<<<nb_k, 256, 0, c->stream>>>(a);
+    dim3 grid(nb_k, (unsigned)c->replicas);
+    if (c->layout == LAY_ROW8) k_map_update<LAY_ROW8><<<grid, 256, 0, c->stream>>>(a);
+    else if (c->layout == LAY_ROW2) k_map_update<LAY_ROW2><<<grid, 256, 0, c->stream>>>(a);
+    else k_map_update<LAY_P16><<<grid, 256, 0, c->stream>>>(a);
+    long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * m : nullptr;
+    k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ, trow, 0);
+    c->launches += 4;
+    IC_CUDA(cudaGetLastError());
+    c->sweep += 1;
+  }
+  return IC_OK;
+}
+
+// ---- drop observable and snapshots (Fig. 7) ------------------------------------------------------------
+extern "C" size_t ic_cluster_scratch_bytes(int L) {
+  if (L < 4 || L > 32768 || (L & (L - 1))) return 0;
+  return (size_t)L * L * 8 + 256;
+}
+
+extern "C" int ic_largest_cluster(ic_ctx* c, int replica, int which, void* d_scratch, size_t scratch_bytes, int64_t* h_out2) {
+  if (!c || !h_out2) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas || !small_index_ok(c)) return IC_ERR_SIZE;
+  if (which < 0 || which > 2) return IC_ERR_PARAM;
+  if (!d_scratch || scratch_bytes < ic_cluster_scratch_bytes(c->L) || ((uintptr_t)d_scratch & 255) != 0) return IC_ERR_WORKSPACE;
+  int* parent = (int*)d_scratch; int* size = parent + c->N; long long* out2 = (long long*)(size + c->N);
+  const LatView lat{c->lattice + (long long)replica * c->lat_stride, c->L, c->logL};
+  const int nb = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);
+  IC_CUDA(cudaMemsetAsync(out2, 0, 16, c->stream));
+  if (c->layout == LAY_ROW8) k_cc_init<LAY_ROW8><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
+  else if (c->layout == LAY_ROW2) k_cc_init<LAY_ROW2><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
+  else k_cc_init<LAY_P16><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
+  k_cc_link<<<nb, 256, 0, c->stream>>>(c->L, c->logL, parent);
+  k_cc_count<<<nb, 256, 0, c->stream>>>(c->N, parent, size);
+  k_cc_max<<<nb, 256, 0, c->stream>>>(c->N, size, out2);
+  c->launches += 4;
+  IC_CUDA(cudaGetLastError());
+  long long h[2];
+  IC_CUDA(cudaMemcpyAsync(h, out2, 16, cudaMemcpyDeviceToHost, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  h_out2[0] = h[0]; h_out2[1] = h[1];
+  return IC_OK;
+}
+
+// Snapshot of one lattice copy as a binary PPM (P6) written from host memory: S=+1 red, S=-1 blue, sigma=+1 white, sigma=-1 dark grey.
+extern "C" int ic_snapshot_ppm(ic_ctx* c, int replica, const char* path) {
+  if (!c || !path) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  std::vector<int8_t> codes((size_t)c->N);
+  int rc = ic_state(c, replica, codes.data());
+  if (rc != IC_OK) return rc;
+  FILE* f = fopen(path, "wb");
+  if (!f) return IC_ERR_PARAM;
+  fprintf(f, "P6\n%d %d\n255\n", c->L, c->L);
+  static const unsigned char pal[4][3] = {{255, 255, 255}, {64, 64, 64}, {220, 30, 30}, {30, 60, 220}};
+  std::vector<unsigned char> row((size_t)c->L * 3);
+  for (int y = 0; y < c->L; ++y) {
+    for (int x = 0; x < c->L; ++x) memcpy(&row[3 * (size_t)x], pal[codes[(size_t)y * c->L + x] & 3], 3);
+    fwrite(row.data(), 1, row.size(), f);
+  }
+  fclose(f);
   return IC_OK;
 }
 

@@ -46,32 +46,13 @@ struct SmemLat {
   __device__ __forceinline__ void store(int x, int y, int, int newc) const { s[(y << logL) + x] = (int8_t)newc; }
 };
 
-// The t-th coupled pair of a phase of schedule S1 (DESIGN.md U4), updated as the paper states it (PAPER.md:64-98):
-// the plain CUDA statement of the method.  thr(class) returns 8*t29 - 1 of the replica.  Adds the accepted move's
-// changes to dn2, dV, dJ, dM, dMs.
+// One coupled-pair update of the pair a = (xa, ya), b = (xb, yb) with the random word w, adj = 1 if b is a
+// neighbour of a (eq. 5) else 0 (eq. 4).  thr(class) returns 8*t29 - 1 of the replica.  Adds the accepted move's changes to
+// dn2, dV, dJ, dM, dMs.
 template <class Lat, class Thr>
-__device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL, int type, int p1, int p2, int phase, uint32_t c2,
-                                                uint32_t c3, uint32_t key0, uint32_t key1, const Thr& thr, long long t,
-                                                int& dn2, int& dV, int& dJ, int& dM, int& dMs) {
+__device__ __forceinline__ void pair_update_core(const Lat& lat, int L, int xa, int ya, int xb, int yb, int adj, uint32_t w, const Thr& thr,
+                                                 int& dn2, int& dV, int& dJ, int& dM, int& dMs) {
   const int mask = L - 1;
-  // --- which pair (schedule S1) and which random word ---------------------------------------------
-  int xa, ya, xb, yb, adj; uint32_t c0, word;
-  if (type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
-    int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
-    xa = 2 * i; ya = 2 * j + phase; xb = xa ^ p1; yb = ya ^ p2; adj = 0;
-    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
-  } else if (p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
-    int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
-    xa = ((p2 + 2 * ((ya + phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
-    c0 = (((uint32_t)xb >> 4) << 2) | ((uint32_t)xb & 3u); word = ((uint32_t)xb >> 2) & 3u;   // addressed by the b-site
-  } else {                           // NEAR, vertical dominoes
-    xa = (int)(t & mask); int jy = (int)(t >> logL);
-    ya = ((p2 + 2 * ((xa + phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
-    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
-  }
-  u32x4 rnd = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
-  uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
-
   // --- proposal: same pair charge q, configuration r of the paper's list ----------
   // all ten sites are loaded up front (independent loads: one memory latency instead of three in a row)
   const int ca = lat.load(xa, ya), cb = lat.load(xb, yb);
@@ -122,6 +103,34 @@ __device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL,
       dMs += (((xa + ya) & 1) ? -dGa : dGa) + (((xb + yb) & 1) ? -dGb : dGb);
     }
   }
+}
+
+// The t-th coupled pair of a phase of schedule S1 (DESIGN.md U4), updated as the paper states it (PAPER.md:64-98):
+// the plain CUDA statement of the method.  thr(class) returns 8*t29 - 1 of the replica.  Adds the accepted move's
+// changes to dn2, dV, dJ, dM, dMs.
+template <class Lat, class Thr>
+__device__ __forceinline__ void ref_pair_update(const Lat& lat, int L, int logL, int type, int p1, int p2, int phase, uint32_t c2,
+                                                uint32_t c3, uint32_t key0, uint32_t key1, const Thr& thr, long long t,
+                                                int& dn2, int& dV, int& dJ, int& dM, int& dMs) {
+  const int mask = L - 1;
+  // --- which pair (schedule S1) and which random word ---------------------------------------------
+  int xa, ya, xb, yb, adj; uint32_t c0, word;
+  if (type == 0) {                 // FAR: a = (even x, y = phase mod 2), b = (x^mx, y^my); eq. (4)
+    int i = (int)(t & ((L >> 1) - 1)), j = (int)(t >> (logL - 1));
+    xa = 2 * i; ya = 2 * j + phase; xb = xa ^ p1; yb = ya ^ p2; adj = 0;
+    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
+  } else if (p1 == 0) {            // NEAR, horizontal dominoes (brick pattern); eq. (5)
+    int i = (int)(t & ((L >> 2) - 1)); ya = (int)(t >> (logL - 2));
+    xa = ((p2 + 2 * ((ya + phase) & 1)) & 3) + 4 * i; xb = (xa + 1) & mask; yb = ya; adj = 1;
+    c0 = (((uint32_t)xb >> 4) << 2) | ((uint32_t)xb & 3u); word = ((uint32_t)xb >> 2) & 3u;   // addressed by the b-site
+  } else {                           // NEAR, vertical dominoes
+    xa = (int)(t & mask); int jy = (int)(t >> logL);
+    ya = ((p2 + 2 * ((xa + phase) & 1)) & 3) + 4 * jy; xb = xa; yb = (ya + 1) & mask; adj = 1;
+    c0 = (((uint32_t)xa >> 4) << 2) | ((uint32_t)xa & 3u); word = ((uint32_t)xa >> 2) & 3u;
+  }
+  u32x4 rnd = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
+  uint32_t w = word == 0 ? rnd.v[0] : word == 1 ? rnd.v[1] : word == 2 ? rnd.v[2] : rnd.v[3];
+  pair_update_core(lat, L, xa, ya, xb, yb, adj, w, thr, dn2, dV, dJ, dM, dMs);
 }
 
 template <int LAY>
