@@ -220,28 +220,32 @@ static int recompute_into_scratch(ic_ctx* c, int replica) {
   const int blocks = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);
   if (c->layout == LAY_ROW8) k_recompute<LAY_ROW8><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
   else if (c->layout == LAY_ROW2) k_recompute<LAY_ROW2><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
-  else k_recompute<LAY_P16><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
+  else k_recompute_p16<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat.base, c->logL, c->d_scratch8);
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
 }
 
-// Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.
-// Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.  `validate`, if given,
-// runs on the host while the copy into the staging buffer is in flight; a non-zero result leaves the lattice untouched.
-template <class F>
-static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, F validate) {
+// Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.  With `validate` the
+// codes are first checked on the device in the staging buffer (every code in 0..3, sum S == Q: eq. 2); a
+// rejected lattice leaves the replica untouched.
+static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, bool validate) {
   char* lat = c->lattice + (long long)replica * c->lat_stride;
-  if (c->layout == LAY_ROW8) {
-    int v = validate();
-    if (v != IC_OK) return v;
-    IC_CUDA(cudaMemcpyAsync(lat, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
-  } else {
-    IC_CUDA(cudaMemcpyAsync(c->d_stage, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
-    int v = validate();
-    if (v != IC_OK) { cudaStreamSynchronize(c->stream); return v; }   // h_codes is the caller's again
-    const long long n16 = c->N / 16;
-    const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
+  const long long n16 = c->N / 16;
+  const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
+  IC_CUDA(cudaMemcpyAsync(c->d_stage, h_codes, (size_t)c->N, cudaMemcpyHostToDevice, c->stream));
+  if (validate) {
+    IC_CUDA(cudaMemsetAsync(c->d_scratch8, 0, 64, c->stream));
+    k_validate_codes<<<blocks, 256, 0, c->stream>>>(c->d_stage, n16, c->d_scratch8);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+    long long h[2];
+    IC_CUDA(cudaMemcpyAsync(h, c->d_scratch8, 16, cudaMemcpyDeviceToHost, c->stream));
+    IC_CUDA(cudaStreamSynchronize(c->stream));
+    if (h[0] != 0 || h[1] != c->Q) return IC_ERR_CHARGE;
+  }
+  if (c->layout == LAY_ROW8) IC_CUDA(cudaMemcpyAsync(lat, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToDevice, c->stream));
+  else {
     if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
     else k_codes_to_p16<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint8_t*)lat, c->logL);
     c->launches++;
@@ -253,9 +257,6 @@ static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, F validat
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
-}
-static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes) {
-  return upload_state(c, replica, h_codes, [] { return (int)IC_OK; });
 }
 
 extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, double J, uint64_t seed, int replicas,
@@ -315,7 +316,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   const long long nplus = c->Q > 0 ? c->Q : 0, nminus = c->Q < 0 ? -c->Q : 0;
   for (int r = 0; r < replicas; ++r) {
     stage1_init(codes.data(), c->N, nplus, nminus, seed, r);
-    int rc = upload_state(c, r, codes.data());
+    int rc = upload_state(c, r, codes.data(), false);
     if (rc != IC_OK) return fail(rc);
     e = cudaStreamSynchronize(c->stream);   // codes is reused for the next replica
     if (e != cudaSuccess) return fail(cuda_fail(e, "cudaStreamSynchronize(init)"));
@@ -341,7 +342,7 @@ extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nm
   if (nplus < 0 || nminus < 0 || nplus + nminus > c->N || nplus - nminus != c->Q) return IC_ERR_CHARGE;
   std::vector<int8_t> codes((size_t)c->N);
   stage1_init(codes.data(), c->N, nplus, nminus, c->seed, replica);
-  int rc = upload_state(c, replica, codes.data());
+  int rc = upload_state(c, replica, codes.data(), false);
   if (rc != IC_OK) return rc;
   IC_CUDA(cudaStreamSynchronize(c->stream));
   return IC_OK;
@@ -350,38 +351,7 @@ extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nm
 extern "C" int ic_set_state(ic_ctx* c, int replica, const int8_t* h_codes) {
   if (!c || !h_codes) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
-  // every code in 0..3 and sum S == Q (eq. 2), eight sites at a time: bit1 = charge, bit0 = sign; on several host
-  // threads, while the copy into the staging buffer is under way
-  auto validate = [&]() -> int {
-    const long long N = c->N;   // N >= 16 and a multiple of 8
-    unsigned hw = std::thread::hardware_concurrency();
-    const int nth = N < (1 << 20) ? 1 : (int)std::max(1u, std::min(hw ? hw : 1u, 16u));
-    std::vector<long long> nch(nth, 0), nneg(nth, 0); std::vector<uint64_t> bad(nth, 0);
-    auto scan = [&](int t) {
-      const long long lo = (N / 8 * t / nth) * 8, hi = (N / 8 * (t + 1) / nth) * 8;
-      long long a = 0, b = 0; uint64_t x = 0;
-      for (long long i = lo; i < hi; i += 8) {
-        uint64_t v; memcpy(&v, h_codes + i, 8);
-        x |= v & 0xFCFCFCFCFCFCFCFCull;
-        const uint64_t ch = (v >> 1) & 0x0101010101010101ull;
-        a += __builtin_popcountll(ch);
-        b += __builtin_popcountll(ch & v);
-      }
-      nch[t] = a; nneg[t] = b; bad[t] = x;
-    };
-    if (nth == 1) scan(0);
-    else {
-      std::vector<std::thread> th;
-      for (int t = 0; t < nth; ++t) th.emplace_back(scan, t);
-      for (auto& t : th) t.join();
-    }
-    long long A = 0, B = 0; uint64_t X = 0;
-    for (int t = 0; t < nth; ++t) { A += nch[t]; B += nneg[t]; X |= bad[t]; }
-    if (X) return IC_ERR_CHARGE;
-    if ((A - B) - B != c->Q) return IC_ERR_CHARGE;
-    return IC_OK;
-  };
-  int rc = upload_state(c, replica, h_codes, validate);
+  int rc = upload_state(c, replica, h_codes, true);
   if (rc != IC_OK) return rc;
   IC_CUDA(cudaStreamSynchronize(c->stream));   // h_codes may be pageable and is the caller's to reuse
   return IC_OK;

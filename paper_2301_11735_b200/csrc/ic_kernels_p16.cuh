@@ -309,4 +309,81 @@ __global__ void __launch_bounds__(256) k_p16_to_codes(const uint8_t* lat, int8_t
   }
 }
 
+// Full recomputation of (n2, bV, bJ, M, Ms, Q) from eq. (3) on the tiled layout: one thread per 16-byte
+// plane vector, bit logic on the (f, g) bytes.  A site is a charge iff f == g (S = f + g - 1), else a spin (sigma = f - g);
+// for a bond (i, j): S_i S_j = +-1 iff both are charges (sign: f_i == f_j), sigma_i sigma_j = +-1 iff both are spins.
+// Every site owns its +x and +y bond: the +x neighbour of plane kx is plane kx+1 (plane 0 one column on for kx = 3), the
+// +y neighbour of row ky is row ky+1 (row 0 of the next quad for ky = 3).  out8 must be zeroed before the launch.
+__global__ void __launch_bounds__(256) k_recompute_p16(const uint8_t* lat, int logL, long long* out8) {
+  const int lw = logL - 2, W = 1 << lw, ls = p16_logseg(lw), SEGL = 1 << ls;
+  const long long nvec = ((long long)1 << (2 * logL)) >> 4;
+  long long acc[6] = {0, 0, 0, 0, 0, 0};
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nvec; t += (long long)gridDim.x * blockDim.x) {
+    // t = ((Y * 16 + row) * (W / 16)) + chunk
+    const int chunk = (int)(t & ((W >> 4) - 1));
+    const int row = (int)(t >> (lw - 4)) & 15, Y = (int)(t >> lw);
+    const int ky = row >> 2, kx = row & 3, X0 = chunk << 4;
+    const int seg = X0 >> ls, xo = X0 & (SEGL - 1);
+    const V16 v = ld16(lat + p16_row(lw, ky, kx, Y, seg) + xo);
+    V16 rgt;
+    if (kx < 3) rgt = ld16(lat + p16_row(lw, ky, kx + 1, Y, seg) + xo);
+    else {
+      const int Xn = (X0 + 16) & (W - 1);
+      rgt = shift_down(ld16(lat + p16_row(lw, ky, 0, Y, seg) + xo), lat[p16_row(lw, ky, 0, Y, Xn >> ls) + (Xn & (SEGL - 1))]);
+    }
+    const V16 dwn = ky < 3 ? ld16(lat + p16_row(lw, ky + 1, kx, Y, seg) + xo) : ld16(lat + p16_row(lw, 0, kx, (Y + 1) & (W - 1), seg) + xo);
+    int n2 = 0, bV = 0, bJ = 0, nf = 0, ng = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const uint32_t m = 0x01010101u;
+      const uint32_t f = v.w[k] & m, g = (v.w[k] >> 3) & m, ch = ~(f ^ g) & m;
+      nf += __popc(f); ng += __popc(g); n2 += __popc(ch);
+#pragma unroll
+      for (int dir = 0; dir < 2; ++dir) {
+        const uint32_t u = dir ? dwn.w[k] : rgt.w[k];
+        const uint32_t fu = u & m, gu = (u >> 3) & m, chu = ~(fu ^ gu) & m, same = ~(f ^ fu) & m;
+        const uint32_t cc = ch & chu, ss = ~ch & ~chu & m;
+        bV += __popc(cc & same) - __popc(cc & ~same);
+        bJ += __popc(ss & same) - __popc(ss & ~same);
+      }
+    }
+    const int Mv = nf - ng;
+    acc[0] += n2; acc[1] += bV; acc[2] += bJ; acc[3] += Mv; acc[4] += ((kx + ky) & 1) ? -Mv : Mv; acc[5] += nf + ng - 16;
+  }
+  __shared__ long long red[6][8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    long long q = acc[k];
+    for (int o = 16; o > 0; o >>= 1) q += __shfl_down_sync(0xFFFFFFFFu, q, o);
+    if (lane == 0) red[k][warp] = q;
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    long long q = 0;
+    for (int wv = 0; wv < 8; ++wv) q += red[threadIdx.x][wv];
+    atomicAdd((unsigned long long*)&out8[threadIdx.x], (unsigned long long)q);
+  }
+}
+
+// Validation of a lattice in public byte codes (ic_set_state): out2[0] = number of bytes outside 0..3, out2[1] = sum S.
+__global__ void __launch_bounds__(256) k_validate_codes(const int8_t* codes, long long n16, long long* out2) {
+  long long bad = 0, q = 0;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n16; t += (long long)gridDim.x * blockDim.x) {
+    const uint4 v = reinterpret_cast<const uint4*>(codes)[t];
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      bad += (w[k] & 0xFCFCFCFCu) != 0u;
+      const uint32_t ch = (w[k] >> 1) & 0x01010101u;          // bit1 = charge, bit0 = negative
+      q += __popc(ch) - 2 * __popc(ch & w[k]);
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) { bad += __shfl_down_sync(0xFFFFFFFFu, bad, o); q += __shfl_down_sync(0xFFFFFFFFu, q, o); }
+  if ((threadIdx.x & 31) == 0) {
+    if (bad) atomicAdd((unsigned long long*)&out2[0], (unsigned long long)bad);
+    if (q) atomicAdd((unsigned long long*)&out2[1], (unsigned long long)q);
+  }
+}
+
 }  // namespace ic
