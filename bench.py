@@ -30,13 +30,36 @@ METRIC = "coupled-pair updates/ns on 1 B200 and % of HBM roofline (L=16384)"
 UNIT = "pair-updates/ns"
 B_ALG_PER_PAIR = {8: 4.0, 2: 1.0}     # bytes: every site once in, once out per sweep
 B_2PASS_PER_PAIR = {8: 8.0, 2: 2.0}   # two data-dependent phases, each one read + one write of the lattice
-# dram__bytes_read.sum + dram__bytes_write.sum per phase launch from the committed `ncu --set full` capture of this very
-# command (profiles/r01e.md: 268.6 MB read + 94.0 MB written, mean over the FAR / NEAR-H / NEAR-V launches); the
-# algorithmic figure is 268.4 MB, the two-pass floor (read all, write the active half) 402.7 MB
-PROFILED_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 362.6e6}
-# warp instructions per 32 pair updates = lane instructions per pair update of the phase kernels, same capture (mean of the
-# three kernel types); issue peak = 148 SMs x 4 sub-partitions x 32 lanes x SM clock
-PROFILED_INSTR_PER_PAIR = {("C5", 8): 41.3}
+
+
+def csrc_sha16():
+    """Hash of the kernel sources: a profile summary under profiles/ belongs to exactly one state of csrc/."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2301_11735_b200", "csrc", "*"))):
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def profiled(config, bits):
+    """ncu-derived figures of the dominant kernel (dram bytes and warp instructions per launch) from the newest
+    profiles/*_summary.csv written for this config; they are reported only while csrc/ still hashes to the state that was
+    profiled, otherwise roofline.traffic is null (a stale capture is not a measurement of this build)."""
+    import glob
+    best = None
+    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_summary.csv"))):
+        kv = {}
+        for ln in open(f).read().splitlines()[1:]:
+            if "," in ln:
+                k, v = ln.split(",", 1)
+                kv[k.strip()] = v.strip()
+        if kv.get("config") == config and int(kv.get("bits", "8")) == bits:
+            best = kv
+    if not best:
+        return None
+    best["stale"] = best.get("source_sha16") != csrc_sha16()
+    return best
 
 
 def measured_peaks():
@@ -188,6 +211,7 @@ def main():
     import torch.distributed as dist
 
     import paper_2301_11735_b200 as ic
+    from paper_2301_11735_b200 import shard
 
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device"
@@ -229,10 +253,7 @@ def main():
     ms = ev0.elapsed_time(ev1)
     launches = sim.launch_count - l0
     clocks = sampler.stop()
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = shard.max_over_ranks(ms)                      # a multi-rank time is the slowest rank's
     value = world * pairs_per_step * args.steps / (ms * 1e6)
 
     # invariants after the timed region: eq. (2) and incremental == recomputed integers
@@ -240,6 +261,12 @@ def main():
     for r in range(min(reps, 2)):
         assert list(sim.debug_recompute(r)) == [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")], "integers drifted"
         assert obs[r]["Q"] == sim.Q
+    # the job's lattice copies are the world * reps global replicas, dealt round-robin (shard.replica_shard); the one
+    # exchange of the whole job is this gather of about 100 B per replica
+    mine = shard.replica_shard(world * reps, rank, world)
+    all_obs = shard.gather_observables({g: {k: obs[i][k] for k in ("Q", "nmeas", "n2", "bV", "bJ", "M", "Ms")} for i, g in enumerate(mine)},
+                                       world * reps)
+    assert all(o["Q"] == sim.Q and o["nmeas"] == obs[0]["nmeas"] for o in all_obs), "a rank lost charge or sweeps"
 
     # ---- end to end through the C ABI with HOST buffers ----------------------------------------------------------------
     e2e = None
@@ -260,10 +287,8 @@ def main():
             o = sim.observables()                     # D2H of the step's observables
         barrier()
         dt = time.perf_counter() - t0
-        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * pairs_per_step * e2e_steps / (float(t.item()) * 1e9), "unit": UNIT,
+        dt = shard.max_over_ranks(dt)
+        e2e = {"value": world * pairs_per_step * e2e_steps / (dt * 1e9), "unit": UNIT,
                "h2d_bytes_per_step": reps * N + 8 * reps, "d2h_bytes_per_step": reps * N + 128 * reps, "steps": e2e_steps,
                "path": "ic_set_state(pinned host) -> ic_sweep -> ic_state(pinned host) + ic_observables"}
 
@@ -274,19 +299,24 @@ def main():
     pairs_per_launch = reps * N // 4
     ach = B_ALG_PER_PAIR[bits] * pairs_per_launch / (avg_ms * 1e6)
     ach2 = B_2PASS_PER_PAIR[bits] * pairs_per_launch / (avg_ms * 1e6)
+    prof = profiled(args.config, bits) if world == 1 else None
     roofline = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get((args.config, bits)) if world == 1 and reps == 1 else None,
+                "traffic": float(prof["dram_bytes_per_launch"]) if prof and not prof["stale"] else None,
+                "traffic_source": (f"profiles/{prof['profile']}_summary.csv" + (" (stale: csrc/ changed since that capture)" if prof["stale"] else "")) if prof else None,
                 "kernel": "phase kernel (one of the two phases of a sweep)", "avg_launch_ms": avg_ms, "peak_source": peak_src,
                 "bytes_per_pair_algorithmic": B_ALG_PER_PAIR[bits],
                 "two_pass": {"bytes_per_pair": B_2PASS_PER_PAIR[bits], "achieved": ach2, "frac": ach2 / peak}}
 
-    ipp = PROFILED_INSTR_PER_PAIR.get((args.config, bits)) if world == 1 and reps == 1 else None
-    if ipp:
+    if prof and not prof["stale"]:
+        ipp = float(prof["instructions_per_pair"])
         mhz = clocks.get("sm_mhz") or 1965.0
-        issue_peak = 148 * 4 * 32 * mhz * 1e6
-        roofline["issue"] = {"bound": "alu", "what": "the path is bound by instruction issue / the integer ALU pipe, not by HBM",
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        issue_peak = sms * 4 * 32 * mhz * 1e6       # one warp instruction per cycle and sub-partition
+        roofline["issue"] = {"what": "lane-instructions issued per second against one warp instruction per cycle and SM sub-partition; "
+                                     "the capture shows the shared-memory data pipe as the busiest unit",
                              "achieved": value * 1e9 * ipp, "peak": issue_peak, "unit": "lane-instructions/s",
-                             "frac": value * 1e9 * ipp / issue_peak, "instructions_per_pair": ipp}
+                             "frac": value * 1e9 * ipp / issue_peak, "instructions_per_pair": ipp, "sm_count": sms,
+                             "lsu_data_pipe_pct_in_capture": float(prof.get("lsu_data_pipe_wavefronts_pct", "nan"))}
     out = None
     if rank == 0:
         out = {
