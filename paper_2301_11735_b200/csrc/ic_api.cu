@@ -220,7 +220,8 @@ static int recompute_into_scratch(ic_ctx* c, int replica) {
   const int blocks = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);
   if (c->layout == LAY_ROW8) k_recompute<LAY_ROW8><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
   else if (c->layout == LAY_ROW2) k_recompute<LAY_ROW2><<<blocks, 256, 0, c->stream>>>(lat, c->d_scratch8);
-  else k_recompute_p16<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat.base, c->logL, c->d_scratch8);
+  else if (c->layout == LAY_P16) k_recompute_p16<8><<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat.base, c->logL, c->d_scratch8);
+  else k_recompute_p16<2><<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat.base, c->logL, c->d_scratch8);
   c->launches++;
   IC_CUDA(cudaGetLastError());
   return IC_OK;
@@ -247,6 +248,7 @@ static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, bool vali
   if (c->layout == LAY_ROW8) IC_CUDA(cudaMemcpyAsync(lat, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToDevice, c->stream));
   else {
     if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
+    else if (c->layout == LAY_P2) k_codes_to_p2<<<std::max(1, blocks / 4), 256, 0, c->stream>>>(c->d_stage, (uint8_t*)lat, c->logL);
     else k_codes_to_p16<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint8_t*)lat, c->logL);
     c->launches++;
     IC_CUDA(cudaGetLastError());
@@ -272,7 +274,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   if (!c) return IC_ERR_NULL;
   c->L = L; c->logL = 0; while ((1 << c->logL) < L) c->logL++;
   c->replicas = replicas; c->bits = bits; c->variant = 0;
-  c->layout = bits == 2 ? LAY_ROW2 : (L >= 64 ? LAY_P16 : LAY_ROW8);
+  c->layout = bits == 2 ? (L >= 128 ? LAY_P2 : LAY_ROW2) : (L >= 64 ? LAY_P16 : LAY_ROW8);
   c->N = (long long)L * L; c->Q = std::llround(n * (double)c->N);
   c->n = n; c->delta = delta; c->V = V; c->J = J; c->seed = seed; c->sweep = 0;
   c->stream = (cudaStream_t)cuda_stream;
@@ -367,6 +369,7 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
     const long long n16 = c->N / 16;
     const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
     if (c->layout == LAY_ROW2) k_unpack2<<<blocks, 256, 0, c->stream>>>((const uint32_t*)lat, c->d_stage, n16);
+    else if (c->layout == LAY_P2) k_p2_to_codes<<<std::max(1, blocks / 4), 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
     else k_p16_to_codes<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
     c->launches++;
     IC_CUDA(cudaGetLastError());
@@ -393,6 +396,7 @@ static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
   dim3 grid((unsigned)((npairs + 255) / 256), (unsigned)c->replicas);
   if (c->layout == LAY_ROW8) IC_CUDA(launch_pdl(k_ref_phase<LAY_ROW8>, grid, dim3(256), 0, c->stream, a));
   else if (c->layout == LAY_ROW2) IC_CUDA(launch_pdl(k_ref_phase<LAY_ROW2>, grid, dim3(256), 0, c->stream, a));
+  else if (c->layout == LAY_P2) IC_CUDA(launch_pdl(k_ref_phase<LAY_P2>, grid, dim3(256), 0, c->stream, a));
   else IC_CUDA(launch_pdl(k_ref_phase<LAY_P16>, grid, dim3(256), 0, c->stream, a));
   c->launches++;
   return IC_OK;
@@ -423,18 +427,22 @@ static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
 }
 
 // Staged kernels on LAY_P16, L >= 2048: one persistent block per SM, TMA-staged regions (ic_kernels_staged.cuh).
-template <int TYPE, int CW>
-static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
-  using C = StagedCfg<TYPE>;
+template <int TYPE, int CW, int BITS>
+static int launch_staged_bits(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
+  using C = StagedCfg<TYPE, BITS>;
   static bool configured[64] = {};   // per instantiation and per device: the attribute belongs to the device's copy of the kernel
   if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
-    IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW, BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     if (c->device >= 0 && c->device < 64) configured[c->device] = true;
   }
-  IC_CUDA(launch_pdl(k_staged_phase<TYPE, CW>, grid, dim3(ST_THREADS), (size_t)C::SMEM_BYTES, c->stream, a));
+  IC_CUDA(launch_pdl(k_staged_phase<TYPE, CW, BITS>, grid, dim3(ST_THREADS), (size_t)C::SMEM_BYTES, c->stream, a));
   return IC_OK;
 }
-static bool staged_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L >= 4 * ST_SEG; }
+template <int TYPE, int CW>
+static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
+  return c->layout == LAY_P2 ? launch_staged_bits<TYPE, CW, 2>(c, a, grid) : launch_staged_bits<TYPE, CW, 8>(c, a, grid);
+}
+static bool staged_ok(const ic_ctx* c) { return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= 4 * ST_SEG; }
 static bool tiled_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L <= 4 * ST_SEG; }   // one tile per row quad
 static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
   const long long ntasks = ((long long)(c->L / 4) * (c->L / 4 / ST_SEG)) / 2;
@@ -626,6 +634,7 @@ extern "C" int ic_sweep_maps(ic_ctx* c, const double* h_T, int64_t nmaps, int64_
     dim3 grid(nb_k, (unsigned)c->replicas);
     if (c->layout == LAY_ROW8) k_map_update<LAY_ROW8><<<grid, 256, 0, c->stream>>>(a);
     else if (c->layout == LAY_ROW2) k_map_update<LAY_ROW2><<<grid, 256, 0, c->stream>>>(a);
+    else if (c->layout == LAY_P2) k_map_update<LAY_P2><<<grid, 256, 0, c->stream>>>(a);
     else k_map_update<LAY_P16><<<grid, 256, 0, c->stream>>>(a);
     long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * m : nullptr;
     k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ, trow, 0);
@@ -653,6 +662,7 @@ extern "C" int ic_largest_cluster(ic_ctx* c, int replica, int which, void* d_scr
   IC_CUDA(cudaMemsetAsync(out2, 0, 16, c->stream));
   if (c->layout == LAY_ROW8) k_cc_init<LAY_ROW8><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
   else if (c->layout == LAY_ROW2) k_cc_init<LAY_ROW2><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
+  else if (c->layout == LAY_P2) k_cc_init<LAY_P2><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
   else k_cc_init<LAY_P16><<<nb, 256, 0, c->stream>>>(lat, which, parent, size);
   k_cc_link<<<nb, 256, 0, c->stream>>>(c->L, c->logL, parent);
   k_cc_count<<<nb, 256, 0, c->stream>>>(c->N, parent, size);

@@ -65,10 +65,15 @@ IC_HD int sg_of(int c) { return (c & 2) ? 0 : 1 - 2 * (c & 1); }
 //         a tile with the plane rows of the lattice row above and below is ONE contiguous piece (one bulk copy).  Byte e = f | g<<3 with (f,g) = sigma+ (1,0), sigma- (0,1),
 //         S+ (1,1), S- (0,0), so that the byte-wise sum of the four neighbour bytes is F | G<<3 with
 //         sum S = F+G-4,  sum sigma = F-G                                          (8 bits/site, L >= 64)
-// Every phase of schedule S1 updates whole plane rows of P16, so the kernels work on dense 16-byte vectors, and a
-// tile (8 KB at SEGL = 512) plus its neighbour rows is what one bulk copy stages in shared memory.
+//   P2    two bits per site, the tiles and plane rows of P16 with 16 plane sites per 32-bit word       (2 bits/site, L >= 128)
+//         (a plane row of SEGL sites is SEGL/4 bytes, every byte offset of P16 divided by 4).  Site k = 4j + m of a word
+//         keeps f at bit 8m + 2j and g at bit (8m + 2j + 3) mod 32, so that the four bytes f | g<<3 of the sites 4j .. 4j+3
+//         are rotr(word, 2j) & 0x09090909: a word widens to the 16-byte vector the P16 arithmetic works on in
+//         1 + 3 x 2 instructions and packs back in 5 (the residues {0,3}, {2,5}, {4,7}, {6,1} tile Z_8).
+// Every phase of schedule S1 updates whole plane rows of P16 / P2, so the kernels work on dense 16-site vectors, and a
+// tile (8 KB at SEGL = 512; 2 KB in P2) plus its neighbour rows is what one bulk copy stages in shared memory.
 // ---------------------------------------------------------------------------------------------------
-enum Layout : int { LAY_ROW8 = 0, LAY_ROW2 = 1, LAY_P16 = 2 };
+enum Layout : int { LAY_ROW8 = 0, LAY_ROW2 = 1, LAY_P16 = 2, LAY_P2 = 3 };
 
 IC_HD int e_of_code(int c) { return (~c & 1) | (((c ^ (c >> 1)) & 1) << 3); }
 IC_HD int code_of_e(int e) { int b0 = ~e & 1; return b0 | ((((e >> 3) ^ b0) & 1) << 1); }
@@ -85,6 +90,16 @@ IC_HD long long p16_site(int lw, int x, int y) {
   return p16_row(lw, y & 3, x & 3, y >> 2, X >> ls) + (X & ((1 << ls) - 1));
 }
 
+// P2 words: bit position of site k's f inside its word; its g sits three bits on (mod 32)
+IC_HD int p2_shift(int k) { return 8 * (k & 3) + 2 * (k >> 2); }
+IC_HD uint32_t rotr32(uint32_t v, int s) { s &= 31; return s ? (v >> s) | (v << (32 - s)) : v; }
+IC_HD uint32_t rotl32(uint32_t v, int s) { s &= 31; return s ? (v << s) | (v >> (32 - s)) : v; }
+IC_HD int p2_site_e(uint32_t word, int k) { return (int)(rotr32(word, p2_shift(k)) & 9u); }   // byte f | g<<3 of site k
+IC_HD long long p2_word(int lw, int x, int y) {        // byte offset of the word that holds site (x, y)
+  const int ls = p16_logseg(lw), X = x >> 2;
+  return (p16_row(lw, y & 3, x & 3, y >> 2, X >> ls) >> 2) + (((X & ((1 << ls) - 1)) >> 4) << 2);
+}
+
 struct LatView {              // one replica
   char* base;
   int L, logL;
@@ -97,13 +112,19 @@ struct Sites {
   }
   static __device__ __forceinline__ int load(const LatView& v, int x, int y) {
     if (LAY == LAY_P16) return code_of_e(((const uint8_t*)v.base)[p16_offset(v, x, y)]);
+    if (LAY == LAY_P2) return code_of_e(p2_site_e(*(const uint32_t*)(v.base + p2_word(v.logL - 2, x, y)), (x >> 2) & 15));
     const long long i = ((long long)y << v.logL) + x;
     if (LAY == LAY_ROW8) return ((const int8_t*)v.base)[i];
     return (((const uint32_t*)v.base)[i >> 4] >> (2 * (int)(i & 15))) & 3;
   }
-  // Sites written in one phase are distinct; with ROW2 several threads share a word: xor the change in.
+  // Sites written in one phase are distinct; with ROW2 / P2 several threads share a word: xor the change in.
   static __device__ __forceinline__ void store(const LatView& v, int x, int y, int oldc, int newc) {
     if (LAY == LAY_P16) { ((uint8_t*)v.base)[p16_offset(v, x, y)] = (uint8_t)e_of_code(newc); return; }
+    if (LAY == LAY_P2) {
+      const uint32_t d = (uint32_t)(e_of_code(oldc) ^ e_of_code(newc));
+      if (d) atomicXor((uint32_t*)(v.base + p2_word(v.logL - 2, x, y)), rotl32(d, p2_shift((x >> 2) & 15)));
+      return;
+    }
     const long long i = ((long long)y << v.logL) + x;
     if (LAY == LAY_ROW8) ((int8_t*)v.base)[i] = (int8_t)newc;
     else atomicXor(&((uint32_t*)v.base)[i >> 4], (uint32_t)(oldc ^ newc) << (2 * (int)(i & 15)));

@@ -34,6 +34,27 @@ __device__ __forceinline__ V16 ld16(const uint8_t* p) {
 __device__ __forceinline__ void st16(uint8_t* p, const V16& v) {
   *reinterpret_cast<uint4*>(p) = make_uint4(v.w[0], v.w[1], v.w[2], v.w[3]);
 }
+// LAY_P2 (ic_common.cuh): a 32-bit word of 16 sites <-> the 16-byte vector of site bytes f | g<<3
+__device__ __forceinline__ V16 widen2(uint32_t w) {
+  V16 r;
+  r.w[0] = w & 0x09090909u; r.w[1] = __funnelshift_r(w, w, 2) & 0x09090909u;
+  r.w[2] = __funnelshift_r(w, w, 4) & 0x09090909u; r.w[3] = __funnelshift_r(w, w, 6) & 0x09090909u;
+  return r;
+}
+__device__ __forceinline__ uint32_t pack2(const V16& v) {          // bytes must be clean (bits 0 and 3 only)
+  return v.w[0] | __funnelshift_l(v.w[1], v.w[1], 2) | __funnelshift_l(v.w[2], v.w[2], 4) | __funnelshift_l(v.w[3], v.w[3], 6);
+}
+// the vector / the site byte at the P16 byte offset `off` of a lattice in either tiled layout (off = site index in P2)
+template <int BITS>
+__device__ __forceinline__ V16 ldvec(const uint8_t* lat, long long off) {
+  if (BITS == 8) return ld16(lat + off);
+  return widen2(*reinterpret_cast<const uint32_t*>(lat + (off >> 2)));
+}
+template <int BITS>
+__device__ __forceinline__ uint32_t ldsite(const uint8_t* lat, long long off) {
+  if (BITS == 8) return lat[off];
+  return (uint32_t)p2_site_e(*reinterpret_cast<const uint32_t*>(lat + ((off >> 4) << 2)), (int)(off & 15));
+}
 __device__ __forceinline__ V16 add(const V16& a, const V16& b) {   // byte-wise: every byte <= 36, no carries
   V16 r;
 #pragma unroll
@@ -309,11 +330,61 @@ __global__ void __launch_bounds__(256) k_p16_to_codes(const uint8_t* lat, int8_t
   }
 }
 
+// Public byte codes, row-major  <->  P2 words.  One thread per 64 consecutive sites of a row = one word of each of the
+// four planes kx.
+__global__ void __launch_bounds__(256) k_codes_to_p2(const int8_t* codes, uint8_t* lat, int logL) {
+  const int lw = logL - 2, L = 1 << logL;
+  const long long n = ((long long)L * L) >> 6;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(t & ((L >> 6) - 1)), y = (int)(t >> (logL - 6));
+    V16 pl[4];
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+      const uint4 v = reinterpret_cast<const uint4*>(codes)[4 * t + g];
+      uint32_t c[4] = {v.x, v.y, v.z, v.w}, e[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) e[k] = (~c[k] & 0x01010101u) | (((c[k] ^ (c[k] >> 1)) & 0x01010101u) << 3);
+      const uint32_t t0 = __byte_perm(e[0], e[1], 0x5140), t1 = __byte_perm(e[2], e[3], 0x5140);
+      const uint32_t t2 = __byte_perm(e[0], e[1], 0x7362), t3 = __byte_perm(e[2], e[3], 0x7362);
+      pl[0].w[g] = __byte_perm(t0, t1, 0x5410); pl[1].w[g] = __byte_perm(t0, t1, 0x7632);
+      pl[2].w[g] = __byte_perm(t2, t3, 0x5410); pl[3].w[g] = __byte_perm(t2, t3, 0x7632);
+    }
+#pragma unroll
+    for (int kx = 0; kx < 4; ++kx)
+      *reinterpret_cast<uint32_t*>(lat + p2_word(lw, 64 * j + kx, y)) = pack2(pl[kx]);
+  }
+}
+__global__ void __launch_bounds__(256) k_p2_to_codes(const uint8_t* lat, int8_t* codes, int logL) {
+  const int lw = logL - 2, L = 1 << logL;
+  const long long n = ((long long)L * L) >> 6;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(t & ((L >> 6) - 1)), y = (int)(t >> (logL - 6));
+    V16 pl[4];
+#pragma unroll
+    for (int kx = 0; kx < 4; ++kx) pl[kx] = widen2(*reinterpret_cast<const uint32_t*>(lat + p2_word(lw, 64 * j + kx, y)));
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+      const uint32_t p0 = pl[0].w[g], p1 = pl[1].w[g], p2 = pl[2].w[g], p3 = pl[3].w[g];
+      const uint32_t t0 = __byte_perm(p0, p1, 0x5140), t1 = __byte_perm(p2, p3, 0x5140);
+      const uint32_t t2 = __byte_perm(p0, p1, 0x7362), t3 = __byte_perm(p2, p3, 0x7362);
+      const uint32_t e[4] = {__byte_perm(t0, t1, 0x5410), __byte_perm(t0, t1, 0x7632), __byte_perm(t2, t3, 0x5410), __byte_perm(t2, t3, 0x7632)};
+      uint32_t c[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t b0 = ~e[k] & 0x01010101u;
+        c[k] = b0 | ((((e[k] >> 3) ^ b0) & 0x01010101u) << 1);
+      }
+      reinterpret_cast<uint4*>(codes)[4 * t + g] = make_uint4(c[0], c[1], c[2], c[3]);
+    }
+  }
+}
+
 // Full recomputation of (n2, bV, bJ, M, Ms, Q) from eq. (3) on the tiled layout: one thread per 16-byte
 // plane vector, bit logic on the (f, g) bytes.  A site is a charge iff f == g (S = f + g - 1), else a spin (sigma = f - g);
 // for a bond (i, j): S_i S_j = +-1 iff both are charges (sign: f_i == f_j), sigma_i sigma_j = +-1 iff both are spins.
 // Every site owns its +x and +y bond: the +x neighbour of plane kx is plane kx+1 (plane 0 one column on for kx = 3), the
 // +y neighbour of row ky is row ky+1 (row 0 of the next quad for ky = 3).  out8 must be zeroed before the launch.
+template <int BITS>
 __global__ void __launch_bounds__(256) k_recompute_p16(const uint8_t* lat, int logL, long long* out8) {
   const int lw = logL - 2, W = 1 << lw, ls = p16_logseg(lw), SEGL = 1 << ls;
   const long long nvec = ((long long)1 << (2 * logL)) >> 4;
@@ -324,14 +395,14 @@ __global__ void __launch_bounds__(256) k_recompute_p16(const uint8_t* lat, int l
     const int row = (int)(t >> (lw - 4)) & 15, Y = (int)(t >> lw);
     const int ky = row >> 2, kx = row & 3, X0 = chunk << 4;
     const int seg = X0 >> ls, xo = X0 & (SEGL - 1);
-    const V16 v = ld16(lat + p16_row(lw, ky, kx, Y, seg) + xo);
+    const V16 v = ldvec<BITS>(lat, p16_row(lw, ky, kx, Y, seg) + xo);
     V16 rgt;
-    if (kx < 3) rgt = ld16(lat + p16_row(lw, ky, kx + 1, Y, seg) + xo);
+    if (kx < 3) rgt = ldvec<BITS>(lat, p16_row(lw, ky, kx + 1, Y, seg) + xo);
     else {
       const int Xn = (X0 + 16) & (W - 1);
-      rgt = shift_down(ld16(lat + p16_row(lw, ky, 0, Y, seg) + xo), lat[p16_row(lw, ky, 0, Y, Xn >> ls) + (Xn & (SEGL - 1))]);
+      rgt = shift_down(ldvec<BITS>(lat, p16_row(lw, ky, 0, Y, seg) + xo), ldsite<BITS>(lat, p16_row(lw, ky, 0, Y, Xn >> ls) + (Xn & (SEGL - 1))));
     }
-    const V16 dwn = ky < 3 ? ld16(lat + p16_row(lw, ky + 1, kx, Y, seg) + xo) : ld16(lat + p16_row(lw, 0, kx, (Y + 1) & (W - 1), seg) + xo);
+    const V16 dwn = ky < 3 ? ldvec<BITS>(lat, p16_row(lw, ky + 1, kx, Y, seg) + xo) : ldvec<BITS>(lat, p16_row(lw, 0, kx, (Y + 1) & (W - 1), seg) + xo);
     int n2 = 0, bV = 0, bJ = 0, nf = 0, ng = 0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {

@@ -44,12 +44,14 @@ struct SubMeta {
 };
 static_assert(sizeof(SubMeta) == 32, "SubMeta layout");
 
-template <int TYPE>
+template <int TYPE, int BITS>
 struct StagedCfg {
   static constexpr int ROWS = TYPE == PH_NEAR_V ? 28 : 24;          // staged plane rows: (ky_rel + 1) * 4 + kx, ky_rel = -1..4 (5)
-  static constexpr int REGION_BYTES = ROWS * ST_SEG;
-  static constexpr int OFF_HALO = 2 * REGION_BYTES;                 // uint8 [2 regions][left, right][32 rows]
-  static constexpr int OFF_SMETA = OFF_HALO + 128;                  // SubMeta[4]
+  static constexpr int RB = ST_SEG * BITS / 8;                      // bytes of a plane row of a tile: 512 (P16) or 128 (P2)
+  static constexpr int REGION_BYTES = ROWS * RB;
+  static constexpr int HE = BITS == 8 ? 1 : 4;                      // edge entries: the site byte (P16) or the whole word that holds it (P2)
+  static constexpr int OFF_HALO = 2 * REGION_BYTES;                 // [2 regions][left, right][32 rows] edge entries
+  static constexpr int OFF_SMETA = OFF_HALO + 128 * HE;             // SubMeta[4]
   static constexpr int STAGE_BYTES = OFF_SMETA + 128;
   static constexpr int NSTAGE = 2 * ST_GROUPS;                      // slots 2g, 2g+1 belong to consumer group g
   // dynamic shared memory map (byte offsets)
@@ -102,6 +104,20 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
   asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
   return v;
 }
+__device__ __forceinline__ uint32_t lds_u32v(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+// staged lattice data in either tiled layout: the 16-site vector at addr, the site byte just left of a vector (the last
+// site of the word / byte at addr) and just right of it (the first site of the word / byte at addr)
+template <int BITS> __device__ __forceinline__ V16 lds_vec(uint32_t addr) { return BITS == 8 ? lds_v16(addr) : widen2(lds_u32v(addr)); }
+template <int BITS> __device__ __forceinline__ uint32_t lds_siteL(uint32_t addr) {
+  if (BITS == 8) return lds_u8(addr);
+  const uint32_t w = lds_u32v(addr);
+  return __funnelshift_l(w, w, 2) & 9u;       // site 15: f at bit 30, g at bit 1
+}
+template <int BITS> __device__ __forceinline__ uint32_t lds_siteR(uint32_t addr) { return BITS == 8 ? lds_u8(addr) : (lds_u32v(addr) & 9u); }
 __device__ __forceinline__ uint2 lds_tab64(uint32_t addr) {
   uint2 v;
   asm("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
@@ -221,9 +237,10 @@ __device__ __forceinline__ void st16_left1_tile(uint8_t* row, uint8_t* left, int
 // The phase kernel.  TYPE: PH_FAR / PH_NEAR_H / PH_NEAR_V; CW: word part of the FAR lane permutation.
 // grid = (blocks, replicas), block = 3 groups of 256 consumer threads + 3 producer warps.
 // ---------------------------------------------------------------------------------------------------------------
-template <int TYPE, int CW>
+template <int TYPE, int CW, int BITS>
 __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_constant__ PhaseArgs A) {
-  using C = StagedCfg<TYPE>;
+  using C = StagedCfg<TYPE, BITS>;
+  constexpr int RB = C::RB, HE = C::HE;
   constexpr int SEG = ST_SEG, LOGSEG = ST_LOGSEG, NST = C::NSTAGE;
   extern __shared__ __align__(128) unsigned char smem[];
   const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
@@ -271,7 +288,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     return U ? (rho0 ^ Mrho) : rho0;
   };
   // byte offset of the tile (Y, seg) in the lattice: tiles in the order [seg][Y], 16 plane rows of SEG bytes each
-  auto tile_off = [&](int Y, int seg) -> long long { return (((long long)seg << lw) + Y) << (LOGSEG + 4); };
+  auto tile_off = [&](int Y, int seg) -> long long { return ((((long long)seg << lw) + Y) << 4) * RB; };
   // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n belongs to consumer group g = n % ST_GROUPS
   // and is its k-th task, k = n / ST_GROUPS; it lives in slot 2 g + (k & 1) on lap (k >> 1) & 1.  A slot is thus always
   // drained by the same group and filled in task order, so nobody can wait on a barrier more than one phase away from
@@ -285,7 +302,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     const int kyr = (lane >> 2) - 1, kx = lane & 3;                     // lane = staged row (ky_rel + 1) * 4 + kx
     const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, kyr, kx) : 0;
     const int dY = kyr < 0 ? -1 : kyr > 3 ? 1 : 0;
-    const int rowoff = (((kyr & 3) << 2) | kx) << LOGSEG;
+    const int rowoff = (((kyr & 3) << 2) | kx) * RB;
     // the edge bytes of a task are loaded one task ahead (their latency hides behind the wait for the ring slot)
     auto halo_load = [&](int t, uint32_t (&hl)[2], uint32_t (&hr)[2]) {
       hl[0] = hl[1] = hr[0] = hr[1] = 0u;
@@ -293,8 +310,13 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
 #pragma unroll
         for (int U = 0; U < 2; ++U) {
           const int rho = region_of(t, U), Yq = rho >> lognseg, sg = rho & (nseg - 1), Yr = (Yq + dY) & Wm;
-          if (hf & 1) hl[U] = lat[tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + SEG - 1];
-          if (hf & 2) hr[U] = lat[tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff];
+          if (BITS == 8) {
+            if (hf & 1) hl[U] = lat[tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + SEG - 1];
+            if (hf & 2) hr[U] = lat[tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff];
+          } else {       // the last / first word of the neighbouring tile's plane row
+            if (hf & 1) hl[U] = *reinterpret_cast<const uint32_t*>(lat + tile_off(Yr, (sg - 1) & (nseg - 1)) + rowoff + RB - 4);
+            if (hf & 2) hr[U] = *reinterpret_cast<const uint32_t*>(lat + tile_off(Yr, (sg + 1) & (nseg - 1)) + rowoff);
+          }
         }
       }
     };
@@ -316,13 +338,13 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
           const uint32_t dst = smem_u32(stg + U * C::REGION_BYTES);
           const int Y = Yq[U];
           if (Y != 0 && Y != Wm) {
-            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * SEG, C::REGION_BYTES, full);
+            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * RB, C::REGION_BYTES, full);
           } else if (Y == 0) {
-            bulk_g2s(dst, lat + tile_off(Wm, sg[U]) + 12 * SEG, 4 * SEG, full);
-            bulk_g2s(dst + 4 * SEG, lat + tile_off(0, sg[U]), (C::ROWS - 4) * SEG, full);
+            bulk_g2s(dst, lat + tile_off(Wm, sg[U]) + 12 * RB, 4 * RB, full);
+            bulk_g2s(dst + 4 * RB, lat + tile_off(0, sg[U]), (C::ROWS - 4) * RB, full);
           } else {
-            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * SEG, 20 * SEG, full);
-            bulk_g2s(dst + 20 * SEG, lat + tile_off(0, sg[U]), (C::ROWS - 20) * SEG, full);
+            bulk_g2s(dst, lat + tile_off(Y - 1, sg[U]) + 12 * RB, 20 * RB, full);
+            bulk_g2s(dst + 20 * RB, lat + tile_off(0, sg[U]), (C::ROWS - 20) * RB, full);
           }
         }
       }
@@ -333,24 +355,30 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
         if (TYPE == PH_FAR) {
           const int UP = paired ? (U ^ 1) : U;
           const int ky = A.phase + 2 * half, kyb = ky ^ (my & 3);
-          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((ky * 4) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(Yq[UP], sg[UP]) + ((kyb * 4) << LOGSEG));
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + (ky * 4) * RB);
+          mt.pb = (unsigned long long)(lat + tile_off(Yq[UP], sg[UP]) + (kyb * 4) * RB);
         } else if (TYPE == PH_NEAR_V) {
           const int ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((ky * 4) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(Yb, seg) + ((kyb * 4) << LOGSEG));
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + (ky * 4) * RB);
+          mt.pb = (unsigned long long)(lat + tile_off(Yb, seg) + (kyb * 4) * RB);
         } else {
           const int ka = (A.p2 + 2 * ((half + A.phase) & 1)) & 3, kb = (ka + 1) & 3;
-          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + ((half * 4 + ka) << LOGSEG));
-          mt.pb = (unsigned long long)(lat + tile_off(Y, seg) + ((half * 4 + kb) << LOGSEG));
-          mt.pl = (unsigned long long)(lat + tile_off(Y, (seg - 1) & (nseg - 1)) + ((half * 4 + ka) << LOGSEG) + SEG - 1);
+          mt.pa = (unsigned long long)(lat + tile_off(Y, seg) + (half * 4 + ka) * RB);
+          mt.pb = (unsigned long long)(lat + tile_off(Y, seg) + (half * 4 + kb) * RB);
+          // the last site of the same plane row of the tile to the left: its byte (P16) or the word that holds it (P2)
+          mt.pl = (unsigned long long)(lat + tile_off(Y, (seg - 1) & (nseg - 1)) + (half * 4 + ka) * RB + RB - HE);
         }
         *(reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + sub) = mt;
       }
 #pragma unroll
       for (int U = 0; U < 2; ++U) {
-        if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = (uint8_t)hl[U];
-        if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = (uint8_t)hr[U];
+        if (BITS == 8) {
+          if (hf & 1) stg[C::OFF_HALO + U * 64 + lane] = (uint8_t)hl[U];
+          if (hf & 2) stg[C::OFF_HALO + U * 64 + 32 + lane] = (uint8_t)hr[U];
+        } else {
+          if (hf & 1) reinterpret_cast<uint32_t*>(stg + C::OFF_HALO)[U * 64 + lane] = hl[U];
+          if (hf & 2) reinterpret_cast<uint32_t*>(stg + C::OFF_HALO)[U * 64 + 32 + lane] = hr[U];
+        }
       }
       halo_load(t + tstep, hl, hr);
       __syncwarp();
@@ -365,12 +393,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     const uint32_t cb = ((uint32_t)r | (TAG_UPDATE << 28)) ^ A.rk[1];
     // byte offsets inside a stage buffer: the 16 bytes at plane column Xc of staged row (ky_rel, kx) of region UU,
     // and the bytes just left / right of them (across the tile edge: the side array filled by the producer)
-    auto off = [&](int UU, int kyr, int kx, int Xc) -> int { return UU * C::REGION_BYTES + ((((kyr + 1) << 2) + (kx & 3)) << LOGSEG) + Xc; };
+    auto off = [&](int UU, int kyr, int kx, int Xc) -> int { return UU * C::REGION_BYTES + (((kyr + 1) << 2) + (kx & 3)) * RB + Xc * BITS / 8; };
     auto offL = [&](int UU, int kyr, int kx, int Xc) -> int {
-      return Xc ? off(UU, kyr, kx, Xc) - 1 : C::OFF_HALO + UU * 64 + ((kyr + 1) << 2) + (kx & 3);
+      return Xc ? off(UU, kyr, kx, Xc) - HE : C::OFF_HALO + HE * (UU * 64 + ((kyr + 1) << 2) + (kx & 3));
     };
     auto offR = [&](int UU, int kyr, int kx, int Xc) -> int {
-      return Xc != SEG - 16 ? off(UU, kyr, kx, Xc) + 16 : C::OFF_HALO + UU * 64 + 32 + ((kyr + 1) << 2) + (kx & 3);
+      return Xc != SEG - 16 ? off(UU, kyr, kx, Xc) + 16 * BITS / 8 : C::OFF_HALO + HE * (UU * 64 + 32 + ((kyr + 1) << 2) + (kx & 3));
     };
     // ---- thread-constant offsets of everything the item loads (relative to the stage buffer) --------------------------
     // o[0] a, o[1] b, o[2..] neighbour vectors; h[..] bytes across the vector's edge for the shifted loads
@@ -391,7 +419,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       sh_l = kxa == 0; sh_r = kxb == 3;
       selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));          // byte part of the lane permutation i -> i ^ (mx >> 2 & 15)
       ky_ctr = ky; kxr = kxa;
-      goffa = kxa * SEG + X0; goffb = kxb * SEG + Xb;
+      goffa = (kxa * SEG + X0) * BITS / 8; goffb = (kxb * SEG + Xb) * BITS / 8;
     } else if (TYPE == PH_NEAR_V) {
       const int kx = half + 2 * hi, ky = (A.p2 + 2 * ((half + A.phase) & 1)) & 3;
       sgn = ((half + ky) & 1) ? -1 : 1;
@@ -403,7 +431,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       oh[1] = sh_l ? offL(U, ky + 1, kx + 3, X0) : offR(U, ky + 1, kx + 1, X0);
       oh[2] = oh[3] = 0;
       ky_ctr = ky; kxr = kx;
-      goffa = kx * SEG + X0; goffb = kx * SEG + X0;
+      goffa = (kx * SEG + X0) * BITS / 8; goffb = goffa;
     } else {
       // NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site
       const int ky = half + 2 * hi;
@@ -417,9 +445,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       oh[1] = offL(U, ky, ka + 3, X0); oh[2] = offR(U, ky, kb + 1, X0); oh[3] = 0;
       ky_ctr = ky; kxr = kb;
       left1 = sh_a != 0;
-      goffa = 8 * hi * SEG; goffb = 8 * hi * SEG + X0;                 // plane rows (ky, ka), (ky, kb)
+      goffa = 8 * hi * RB; goffb = 8 * hi * RB + X0 * BITS / 8;        // plane rows (ky, ka), (ky, kb)
     }
-    constexpr int ROW4 = 4 << LOGSEG;                                  // four staged rows = one lattice row up / down
+    constexpr int ROW4 = 4 * RB;                                       // four staged rows = one lattice row up / down
     const uint32_t stg_g = smem0 + C::OFF_STAGE + 2 * g * C::STAGE_BYTES;
     const SubMeta* meta_g = reinterpret_cast<const SubMeta*>(smem + C::OFF_STAGE + 2 * g * C::STAGE_BYTES + C::OFF_SMETA) + sub;
 
@@ -434,35 +462,37 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       uint8_t* gpl = nullptr;
       V16 a, b, ea, eb;
       if (TYPE == PH_FAR) {
-        a = lds_v16(st + oa); b = lds_v16(st + ob);
-        V16 l = lds_v16(st + on[0]);
-        if (sh_l) l = shift_up(l, lds_u8(st + oh[0]));
-        ea = add(add(l, lds_v16(st + on[1])), add(lds_v16(st + oa - ROW4), lds_v16(st + oa + ROW4)));
-        V16 rr = lds_v16(st + on[3]);
-        if (sh_r) rr = shift_down(rr, lds_u8(st + oh[1]));
-        eb = add(add(lds_v16(st + on[2]), rr), add(lds_v16(st + ob - ROW4), lds_v16(st + ob + ROW4)));
+        a = lds_vec<BITS>(st + oa); b = lds_vec<BITS>(st + ob);
+        V16 l = lds_vec<BITS>(st + on[0]);
+        if (sh_l) l = shift_up(l, lds_siteL<BITS>(st + oh[0]));
+        ea = add(add(l, lds_vec<BITS>(st + on[1])), add(lds_vec<BITS>(st + oa - ROW4), lds_vec<BITS>(st + oa + ROW4)));
+        V16 rr = lds_vec<BITS>(st + on[3]);
+        if (sh_r) rr = shift_down(rr, lds_siteR<BITS>(st + oh[1]));
+        eb = add(add(lds_vec<BITS>(st + on[2]), rr), add(lds_vec<BITS>(st + ob - ROW4), lds_vec<BITS>(st + ob + ROW4)));
         b = xor_perm<CW>(b, selb); eb = xor_perm<CW>(eb, selb);          // b into a's lane order (lane i <-> i ^ c)
       } else if (TYPE == PH_NEAR_V) {
-        a = lds_v16(st + oa); b = lds_v16(st + ob);
-        V16 al = lds_v16(st + on[0]), ar = lds_v16(st + on[1]), bl = lds_v16(st + on[2]), br = lds_v16(st + on[3]);
-        if (sh_l) { al = shift_up(al, lds_u8(st + oh[0])); bl = shift_up(bl, lds_u8(st + oh[1])); }
-        if (sh_r) { ar = shift_down(ar, lds_u8(st + oh[0])); br = shift_down(br, lds_u8(st + oh[1])); }
+        a = lds_vec<BITS>(st + oa); b = lds_vec<BITS>(st + ob);
+        V16 al = lds_vec<BITS>(st + on[0]), ar = lds_vec<BITS>(st + on[1]), bl = lds_vec<BITS>(st + on[2]), br = lds_vec<BITS>(st + on[3]);
+        if (sh_l) { al = shift_up(al, lds_siteL<BITS>(st + oh[0])); bl = shift_up(bl, lds_siteL<BITS>(st + oh[1])); }
+        if (sh_r) { ar = shift_down(ar, lds_siteR<BITS>(st + oh[0])); br = shift_down(br, lds_siteR<BITS>(st + oh[1])); }
         // vertical domino: a's lower neighbour is b, b's upper neighbour is a
-        ea = add(add(al, ar), add(lds_v16(st + oa - ROW4), b));
-        eb = add(add(bl, br), add(a, lds_v16(st + ob + ROW4)));
+        ea = add(add(al, ar), add(lds_vec<BITS>(st + oa - ROW4), b));
+        eb = add(add(bl, br), add(a, lds_vec<BITS>(st + ob + ROW4)));
       } else {
-        a = lds_v16(st + oa); b = lds_v16(st + ob);
-        V16 au = lds_v16(st + oa - ROW4), ad = lds_v16(st + oa + ROW4), al = lds_v16(st + on[0]), br = lds_v16(st + on[1]);
+        a = lds_vec<BITS>(st + oa); b = lds_vec<BITS>(st + ob);
+        V16 au = lds_vec<BITS>(st + oa - ROW4), ad = lds_vec<BITS>(st + oa + ROW4), al = lds_vec<BITS>(st + on[0]), br = lds_vec<BITS>(st + on[1]);
         if (sh_a) {
-          a = shift_up(a, lds_u8(st + oh[0]));
-          au = shift_up(au, lds_u8(st + oh[0] + (X0 ? -ROW4 : -4))); ad = shift_up(ad, lds_u8(st + oh[0] + (X0 ? ROW4 : 4)));
+          a = shift_up(a, lds_siteL<BITS>(st + oh[0]));
+          au = shift_up(au, lds_siteL<BITS>(st + oh[0] + (X0 ? -ROW4 : -4 * HE))); ad = shift_up(ad, lds_siteL<BITS>(st + oh[0] + (X0 ? ROW4 : 4 * HE)));
         }
-        if (sh_l) al = shift_up(al, lds_u8(st + oh[1]));
-        if (sh_r) br = shift_down(br, lds_u8(st + oh[2]));
+        if (sh_l) al = shift_up(al, lds_siteL<BITS>(st + oh[1]));
+        if (sh_r) br = shift_down(br, lds_siteR<BITS>(st + oh[2]));
         ea = add(add(al, b), add(au, ad));
-        eb = add(add(a, br), add(lds_v16(st + ob - ROW4), lds_v16(st + ob + ROW4)));
+        eb = add(add(a, br), add(lds_vec<BITS>(st + ob - ROW4), lds_vec<BITS>(st + ob + ROW4)));
         gpl = reinterpret_cast<uint8_t*>(mp->pl) + goffa;
       }
+      V16 a_old;
+      if (BITS == 2 && TYPE == PH_NEAR_H) a_old = a;
       // everything the item needs is in registers: hand the ring slot back to the producers before the long part
       __syncwarp();
       if (lane == 0) mbar_arrive(bar0 + 8 * (NST + s));
@@ -479,9 +509,25 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       }
       if (TYPE == PH_FAR) b = xor_perm<CW>(b, selb);
       sigma_sums(a, aF, aT); sigma_sums(b, bF, bT);
-      st16(gpb, b);
-      if (TYPE == PH_NEAR_H) { if (!left1) st16(gpa + X0, a); else st16_left1_tile(gpa, gpl, X0, a); }
-      else st16(gpa, a);
+      if (BITS == 8) {
+        st16(gpb, b);
+        if (TYPE == PH_NEAR_H) { if (!left1) st16(gpa + X0, a); else st16_left1_tile(gpa, gpl, X0, a); }
+        else st16(gpa, a);
+      } else {
+        *reinterpret_cast<uint32_t*>(gpb) = pack2(b);
+        if (TYPE == PH_NEAR_H && left1) {
+          // the vector holds the sites X0-1 .. X0+14: site X0-1 lives in the word to the left (owned by the neighbouring
+          // lane, or by another block across the tile edge) and site X0+15 of this word is somebody else's, so the
+          // changes are xor-ed in (commutative: no order between the two writers of a word is needed)
+          const V16 d = {{a.w[0] ^ a_old.w[0], a.w[1] ^ a_old.w[1], a.w[2] ^ a_old.w[2], a.w[3] ^ a_old.w[3]}};
+          const uint32_t own = pack2(shift_down(d, 0u)), prev = __funnelshift_l(d.w[0] & 9u, d.w[0] & 9u, 30);
+          uint32_t* wa = reinterpret_cast<uint32_t*>(gpa) + chunk;
+          if (own) atomicXor(wa, own);
+          if (prev) atomicXor(X0 ? wa - 1 : reinterpret_cast<uint32_t*>(gpl), prev);
+        } else {
+          *reinterpret_cast<uint32_t*>(TYPE == PH_NEAR_H ? gpa + X0 / 4 : gpa) = pack2(a);
+        }
+      }
       // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
       const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
       const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;

@@ -86,7 +86,7 @@ def test_schedule_matches_oracle(pkg):
 
 
 def test_stage1_init_matches_oracle(pkg):
-    for (L, n, seed, reps) in [(16, 0.25, 1, 3), (64, 0.1, 2, 2), (64, -0.3, 9, 1), (256, 0.05, 5, 1), (8, 1.0, 3, 1), (8, 0.0, 3, 1)]:
+    for (L, n, seed, reps) in [(16, 0.25, 1, 3), (64, 0.1, 2, 2), (64, -0.3, 9, 1), (256, 0.05, 5, 1), (128, -0.1, 6, 2), (2048, 0.2, 7, 1), (8, 1.0, 3, 1), (8, 0.0, 3, 1)]:
         for bits in (8, 2):
             sim = pkg.Sim(L, n, 0.5, 1.0, 1.0, seed=seed, replicas=reps, bits_per_site=bits)
             Q = sim.Q
@@ -141,9 +141,11 @@ PARITY_CASES = [
     (64, 8, 5, (410, 0), (0.0, 0.5, 1.0), [0.05, 0.5, 1.0, 2.0, 3.2], 60),
     (64, 2, 3, (410, 0), (0.0, 0.5, 1.0), [0.05, 1.0, 3.2], 60),
     (128, 8, 2, (2000, 1000), (1.0, 0.25, 1.0), [0.2, 2.0], 40),
+    (128, 2, 2, (2000, 1000), (1.0, 0.25, 1.0), [0.2, 2.0], 40),   # tiled 2-bit layout: two words per plane row
     (256, 8, 1, (0, 0), (0.2, 1.0, 1.0), [1.0], 30),            # no charges: plain Ising with coupling J/4
     (256, 2, 2, (20000, 20000), (-0.5, 1.0, 2.0), [0.8, 0.3], 30),
     (512, 8, 1, (13107, 0), (0.2, 1.0, 1.0), [1.0], 12),
+    (512, 2, 1, (13107, 20000), (0.2, 1.0, 1.0), [0.9], 12),
 ]
 
 
@@ -357,9 +359,10 @@ def test_staged_kernels_one_block_per_replica(pkg):
 
 
 # ------------------------------------------------------------------------------------------------ kernel variants
-@pytest.mark.parametrize("L,reps,nsweeps,variant", [(64, 3, 64, 2), (128, 2, 64, 2), (256, 2, 48, 2), (1024, 1, 40, 2),
-                                                    (2048, 2, 32, 2), (2048, 2, 48, 3), (4096, 2, 32, 3), (8192, 1, 12, 3)])
-def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant):
+@pytest.mark.parametrize("L,reps,nsweeps,variant,bits", [(64, 3, 64, 2, 8), (128, 2, 64, 2, 8), (256, 2, 48, 2, 8), (1024, 1, 40, 2, 8),
+                                                         (2048, 2, 32, 2, 8), (2048, 2, 48, 3, 8), (4096, 2, 32, 3, 8), (8192, 1, 12, 3, 8),
+                                                         (2048, 2, 64, 3, 2), (4096, 2, 48, 3, 2), (8192, 1, 16, 3, 2)])
+def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant, bits):
     """Variant 2 (tiled, L <= 2048) and variant 3 (TMA-staged, L >= 2048) against variant 1 (one thread per pair) on the
     same device memory layout, sweep by sweep so that many (mx, my) masks, both domino orientations and all four offsets
     are exercised; the reference kernels are themselves compared with the oracle above and (at L <= 256) here."""
@@ -368,8 +371,8 @@ def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant):
     n = (nplus - nminus) / (L * L)
     Ts = [0.4, 1.1, 2.5][:reps]
     codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
-    a = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); a.set_variant(variant)
-    b = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps); b.set_variant(1)
+    a = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps, bits_per_site=bits); a.set_variant(variant)
+    b = pkg.Sim(L, n, 0.3, 1.0, 1.5, seed=seed, replicas=reps, bits_per_site=bits); b.set_variant(1)
     for r in range(reps):
         a.set_state(r, codes[r]); b.set_state(r, codes[r])
     seen = set()
@@ -388,13 +391,15 @@ def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant):
     a.close(); b.close()
 
 
-def test_staged_kernels_against_oracle_l2048(pkg):
-    """Variant 3 (TMA-staged regions) at its smallest size against the oracle: several FAR and NEAR sweeps, 2 replicas."""
+@pytest.mark.parametrize("bits", [8, 2])
+def test_staged_kernels_against_oracle_l2048(pkg, bits):
+    """Variant 3 (TMA-staged regions) at its smallest size against the oracle: several FAR and NEAR sweeps, 2 replicas;
+    both tiled layouts (one byte and two bits per site)."""
     L, seed, nsw = 2048, 77, 6
     nplus, nminus = L * L // 8, L * L // 16
     Ts = [0.7, 1.9]
     codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(2)]
-    sim = pkg.Sim(L, (nplus - nminus) / (L * L), -0.5, 1.0, 2.0, seed=seed, replicas=2); sim.set_variant(3)
+    sim = pkg.Sim(L, (nplus - nminus) / (L * L), -0.5, 1.0, 2.0, seed=seed, replicas=2, bits_per_site=bits); sim.set_variant(3)
     for r in range(2):
         sim.set_state(r, codes[r])
     Ts2 = [1.3, 0.45]                                  # the temperatures change between the calls: new class tables
