@@ -146,9 +146,12 @@ int ic_snapshot_ppm(ic_ctx* ctx, int replica, const char* path);
 
 /* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
  * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels
- * (8 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default there).
+ * (8 or 2 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default there).
  * 4 = resident kernel (L <= 64, any bits_per_site: one block per replica keeps its lattice in shared memory and
  * runs all sweeps of an ic_sweep call in one launch; the default for L <= 64).
+ * 5 = one-launch kernel (8 or 2 bits/site, 128 <= L <= 1024, replicas <= number of SMs: one cooperative launch runs
+ * all sweeps of an ic_sweep call on the whole GPU, the phases separated by a barrier over the replica's blocks; the
+ * default there).
  * IC_ERR_PARAM if the variant cannot run this context's (L, bits_per_site).  All variants produce identical
  * lattices and observables.                                                                           */
 int ic_set_variant(ic_ctx* ctx, int variant);

@@ -18,6 +18,7 @@
 #include "ic_kernels_p16.cuh"
 #include "ic_kernels_staged.cuh"
 #include "ic_kernels_resident.cuh"
+#include "ic_kernels_coop.cuh"
 #include "ic_kernels_extra.cuh"
 
 using namespace ic;
@@ -30,13 +31,14 @@ struct ic_ctx {
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; CoopScratch* d_coop; int8_t* d_stage;
   // host (pinned)
   uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
   std::vector<double>* lastT; bool have_T;
   long long launches;
   int sm_count, device;
+  bool coop_supported;
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -66,6 +68,7 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   b += align256(2 * ST_DESC_ENTRIES * sizeof(uint2));              // move descriptors of the staged kernels
   b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
   b += 256;                                                        // scratch for ic_debug_recompute
+  b += align256((size_t)replicas * sizeof(CoopScratch));           // per-sweep sums and barrier counters of the one-launch kernel
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
   return b;
 }
@@ -286,6 +289,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   c->d_desc32 = (uint2*)p; p += align256(2 * ST_DESC_ENTRIES * sizeof(uint2));
   c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
   c->d_scratch8 = (long long*)p; p += 256;
+  c->d_coop = (CoopScratch*)p; p += align256((size_t)replicas * sizeof(CoopScratch));
   c->d_stage = (int8_t*)p;
   c->h_thr = nullptr; c->h_obs = nullptr; c->thr_copied = nullptr;
 
@@ -311,6 +315,8 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
       return fail(cuda_fail(cudaGetLastError(), "cudaDeviceGetAttribute(multiProcessorCount)"));
     c->sm_count = sms; c->device = dev;
+    int coop = 0;
+    c->coop_supported = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop != 0;
   }
 
   // stage 1 for every replica
@@ -442,6 +448,30 @@ template <int TYPE, int CW>
 static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
   return c->layout == LAY_P2 ? launch_staged_bits<TYPE, CW, 2>(c, a, grid) : launch_staged_bits<TYPE, CW, 8>(c, a, grid);
 }
+// one cooperative launch for all the sweeps of a call: single mid-size lattices (ic_kernels_coop.cuh)
+static bool coop_ok(const ic_ctx* c) {
+  return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= COOP_MIN_L && c->L <= COOP_MAX_L && c->replicas <= c->sm_count && c->coop_supported;
+}
+template <int BITS>
+static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
+  static bool configured[64] = {};
+  if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
+    IC_CUDA(cudaFuncSetAttribute(k_coop_sweeps<BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, COOP_SMEM_BYTES));
+    if (c->device >= 0 && c->device < 64) configured[c->device] = true;
+  }
+  CoopArgs a;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.desc32 = c->d_desc32; a.obs = c->d_obs; a.scratch = c->d_coop; a.trace = (long long*)d_trace;
+  a.lat_stride = c->lat_stride; a.nsweeps = nsweeps; a.sweep0 = c->sweep; a.delta = c->delta; a.V = c->V; a.quarterJ = 0.25 * c->J;
+  a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
+  const long long items = c->N / 16;                                   // four pairs per item, N/4 pairs per phase
+  const long long want = (items + COOP_THREADS - 1) / COOP_THREADS, cap = std::max<long long>(1, c->sm_count / c->replicas);
+  dim3 grid((unsigned)std::min(want, cap), (unsigned)c->replicas);
+  IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
+  void* args[] = {(void*)&a};
+  IC_CUDA(cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(COOP_THREADS), args, (size_t)COOP_SMEM_BYTES, c->stream));
+  c->launches++;
+  return IC_OK;
+}
 static bool staged_ok(const ic_ctx* c) { return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= 4 * ST_SEG; }
 static bool tiled_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L <= 4 * ST_SEG; }   // one tile per row quad
 static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
@@ -512,6 +542,14 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     else k_resident_sweeps<LAY_P16><<<c->replicas, rthreads, 0, c->stream>>>(ra);
     c->launches++;
     IC_CUDA(cudaGetLastError());
+    c->sweep += (uint64_t)nsweeps;
+    return IC_OK;
+  }
+
+  // single mid-size lattices: all the sweeps in one cooperative launch over the whole GPU
+  if (coop_ok(c) && (c->variant == 0 || c->variant == 5)) {
+    int rc = c->layout == LAY_P2 ? launch_coop<2>(c, nsweeps, d_trace) : launch_coop<8>(c, nsweeps, d_trace);
+    if (rc != IC_OK) return rc;
     c->sweep += (uint64_t)nsweeps;
     return IC_OK;
   }
@@ -718,7 +756,8 @@ extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->lau
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {
   if (!c) return IC_ERR_NULL;
-  if (variant < 0 || variant > 4) return IC_ERR_PARAM;
+  if (variant < 0 || variant > 5) return IC_ERR_PARAM;
+  if (variant == 5 && !coop_ok(c)) return IC_ERR_PARAM;
   if (variant == 4 && c->L > RES_MAX_L) return IC_ERR_PARAM;
   if (variant == 2 && !tiled_ok(c)) return IC_ERR_PARAM;
   if (variant == 3 && !staged_ok(c)) return IC_ERR_PARAM;

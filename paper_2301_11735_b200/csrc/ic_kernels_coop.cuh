@@ -1,0 +1,288 @@
+// ic_kernels_coop.cuh -- variant 5: single mid-size lattices (128 <= L <= 1024, config C3 of BASELINE.json) on the tiled
+// layouts LAY_P16 / LAY_P2.
+//
+// A sweep of a 1024 x 1024 lattice is 2 x 262 144 pair updates: a third of a microsecond of arithmetic for the whole chip.
+// With one launch per phase such a run is bound by launch and memory latency, not by any throughput.  Here ONE
+// cooperative launch runs all the sweeps of an ic_sweep call on the whole GPU:
+//   * the lattice stays in global memory (L2-resident: 1 MiB at most); the class tables and the per-lane move descriptors
+//     of the staged kernels sit in shared memory for the whole launch (no table fill per phase);
+//   * an item is FOUR coupled pairs (one 32-bit word of a 16-site plane vector, one Philox block): 65 536 items per phase at
+//     L = 1024 for 148 x 512 threads, so every thread has at most one short item per phase and the phase is one memory
+//     latency + one Philox block + one pairs4 (the item code of the staged kernels) long.  The four lanes of a quad load
+//     the same vectors (shifts and the FAR lane permutation work on whole vectors) and keep their own word;
+//   * the two phases of a sweep are separated by a barrier over the blocks of the replica (a counter in global memory:
+//     red.add + ld.acquire poll); the schedule of every sweep is derived on the device (the Philox call the host makes);
+//   * observables: per-thread sums -> warp REDUX -> block -> int64 atomics into a per-sweep accumulator that is double
+//     buffered by the sweep's parity; thread 0 of the replica's first block folds it after the sweep's second barrier
+//     (U5, the operations of k_fold in the same order) while the other blocks are already in the next sweep.
+// grid = (blocks per replica, replicas), replicas <= number of SMs; cooperative launch (all blocks co-resident).
+#pragma once
+#include "ic_common.cuh"
+#include "ic_kernels_ref.cuh"
+#include "ic_kernels_p16.cuh"
+#include "ic_kernels_staged.cuh"
+
+namespace ic {
+
+constexpr int COOP_THREADS = 512;
+constexpr int COOP_MIN_L = 128, COOP_MAX_L = 1024;
+constexpr int COOP_OFF_THR = 0;                                    // uint32 threshold[THR_STRIDE], packed deltas[THR_STRIDE]
+constexpr int COOP_OFF_DESC = COOP_OFF_THR + THR_STRIDE * 8;       // [2 sweep types] uint2 descriptors [8][28][16]
+constexpr int COOP_SMEM_BYTES = COOP_OFF_DESC + 2 * ST_DESC_SMEM;
+
+struct CoopScratch {            // one per replica, in the workspace; zeroed before every launch
+  long long acc[2][5];          // per-sweep sums (dn2, dV, dJ, M, Ms of the updated sites), buffer = sweep parity
+  unsigned int arrived;         // barrier counter of the replica's blocks (monotonic within a launch)
+  unsigned int pad[11];
+};
+static_assert(sizeof(CoopScratch) == 128, "CoopScratch layout");
+
+struct CoopArgs {
+  void* lattice; const uint2* thr; const uint2* desc32; ReplicaObs* obs; CoopScratch* scratch;
+  long long* trace;              // nullptr or [nsweeps][replicas][6]
+  long long lat_stride, nsweeps;
+  unsigned long long sweep0;
+  double delta, V, quarterJ;
+  int L, logL, replicas;
+  uint32_t key0, key1;
+};
+
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// barrier over the blocks that share `counter`; everything the blocks wrote before it is visible to all of them after it
+__device__ __forceinline__ void coop_barrier(unsigned int* counter, unsigned int target) {
+  __syncthreads();                 // the block's writes happen before thread 0's release (causality order through the barrier)
+  if (threadIdx.x == 0) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+    while (ld_acquire_u32(counter) < target) { }
+  }
+  __syncthreads();
+}
+
+// the four site bytes at plane columns X .. X+3 (X a multiple of 4) of the plane row at site offset `row`
+template <int BITS>
+__device__ __forceinline__ uint32_t ldw(const uint8_t* lat, int row, int X) {
+  if (BITS == 8) return *reinterpret_cast<const uint32_t*>(lat + row + X);
+  const uint32_t w = *reinterpret_cast<const uint32_t*>(lat + ((row + (X & ~15)) >> 2));
+  return __funnelshift_r(w, w, (X >> 1) & 6) & 0x09090909u;             // sites 4j .. 4j+3 of the word: rotr by 2j
+}
+// ... at X + sh .. X + sh + 3, sh in {-1, 0, +1}, periodic in the row of W sites (one tile per row quad)
+template <int BITS>
+__device__ __forceinline__ uint32_t ldw_sh(const uint8_t* lat, int row, int X, int W, int sh) {
+  const uint32_t w = ldw<BITS>(lat, row, X);
+  if (sh < 0) return (w << 8) | ldsite<BITS>(lat, row + ((X - 1) & (W - 1)));
+  if (sh > 0) return (w >> 8) | (ldsite<BITS>(lat, row + ((X + 4) & (W - 1))) << 24);
+  return w;
+}
+
+// stores the four site bytes `w4` (clean: bits 0 and 3) of word j of the vector at X0 of plane row `row`.
+// P2: the four lanes of the quad merge their words and lane j = 0 stores the packed word.
+template <int BITS>
+__device__ __forceinline__ void st_word(uint8_t* lat, int row, int X0, int j, uint32_t w4) {
+  if (BITS == 8) { *reinterpret_cast<uint32_t*>(lat + row + X0 + 4 * j) = w4; return; }
+  // only the quad is named in the mask: at L = 128 the two halves of a warp work on different row classes and may be in
+  // different branches (aligned store / store shifted by one site) when they get here
+  const unsigned qm = 0xFu << ((threadIdx.x & 31) & 28);
+  uint32_t p = __funnelshift_l(w4, w4, 2 * j);
+  p |= __shfl_xor_sync(qm, p, 1);
+  p |= __shfl_xor_sync(qm, p, 2);
+  if (j == 0) *reinterpret_cast<uint32_t*>(lat + ((row + X0) >> 2)) = p;
+}
+// the same for a vector that starts one site to the left (sites X0-1+4j .. X0+2+4j, periodic): bytes cross word borders
+template <int BITS>
+__device__ __forceinline__ void st_word_left1(uint8_t* lat, int row, int X0, int W, int j, uint32_t w4, uint32_t old4) {
+  if (BITS == 8) {
+#pragma unroll
+    for (int m = 0; m < 4; ++m) lat[row + ((X0 - 1 + 4 * j + m) & (W - 1))] = (uint8_t)((w4 >> (8 * m)) & 0xFFu);
+    return;
+  }
+  // P2: xor the changes into the words (two lanes of different quads may share a word; xor commutes)
+  const uint32_t d = w4 ^ old4;
+  if (d == 0u) return;
+  uint32_t own = 0u;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    const uint32_t e = (d >> (8 * m)) & 9u;
+    const int k = 4 * j - 1 + m;                               // site inside the word at X0; -1 = site 15 of the word to the left
+    if (k < 0) { if (e) atomicXor(reinterpret_cast<uint32_t*>(lat + ((row + ((X0 - 16) & (W - 1))) >> 2)), rotl32(e, p2_shift(15))); }
+    else own |= rotl32(e, p2_shift(k));
+  }
+  if (own) atomicXor(reinterpret_cast<uint32_t*>(lat + ((row + X0) >> 2)), own);
+}
+
+template <int BITS>
+__global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs A) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ int s_par[4];
+  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
+  const uint32_t smem0 = smem_u32(smem);
+  {
+    const uint2* src = A.thr + (long long)r * THR_STRIDE;
+    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
+    for (int k = tid; k < THR_STRIDE; k += COOP_THREADS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+    uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
+    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += COOP_THREADS) {
+      const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
+      const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
+      uint2 d = __ldg(&A.desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
+      d.y += smem0 + COOP_OFF_THR;                // low 16 bits: shared-memory address of the class base
+      desc_s[k] = d;
+    }
+  }
+  const int L = A.L, lw = A.logL - 2, W = 1 << lw, Wm = W - 1;
+  const int lognch = lw - 4, nch = 1 << lognch;
+  const int n_items = (W * 4 * nch) * 4;                           // (Y, half, hi, chunk, word)
+  uint8_t* lat = reinterpret_cast<uint8_t*>(A.lattice) + (long long)r * A.lat_stride;
+  CoopScratch* sc = &A.scratch[r];
+  const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
+  const bool folder = blockIdx.x == 0 && tid == 0;
+  ReplicaObs o;
+  if (folder) o = A.obs[r];
+  unsigned int bar_target = 0;
+  __syncthreads();
+
+  for (long long s = 0; s < A.nsweeps; ++s) {
+    const unsigned long long sweep = A.sweep0 + (unsigned long long)s;
+    if (tid == 0) {
+      // U4: parameters of the sweep, the same for all replicas (identical maps for all copies)
+      const u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, A.key0, A.key1);
+      if ((sweep & 1) == 0) { s_par[0] = 0; s_par[1] = (int)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); s_par[2] = (int)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1); }
+      else { s_par[0] = 1; s_par[1] = (int)(z.v[0] & 1u); s_par[2] = (int)(z.v[1] & 3u); }
+    }
+    __syncthreads();
+    const int type = s_par[0], p1 = s_par[1], p2 = s_par[2];
+    const uint32_t s_desc = smem0 + COOP_OFF_DESC + (type ? ST_DESC_SMEM : 0) + (uint32_t)(lane & 15) * 8u;
+    long long* acc = sc->acc[s & 1];
+
+    int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;       // this thread's sums over both phases of the sweep
+    for (int phase = 0; phase < 2; ++phase) {
+      const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
+      for (int it = blockIdx.x * COOP_THREADS + tid; it < n_items; it += gridDim.x * COOP_THREADS) {
+        const int j = it & 3, chunk = (it >> 2) & (nch - 1), hi = (it >> (2 + lognch)) & 1, half = (it >> (3 + lognch)) & 1;
+        const int Y = it >> (4 + lognch), X0 = chunk << 4;
+        uint32_t A4, B4, EA4, EB4, c0;
+        int a3 = 0, sgn, y;
+        const int Xj = X0 + 4 * j;                                      // plane column of the item's first pair
+        auto R = [lw](int ky, int kx, int Yq) -> int { return ((Yq << 4) + (ky << 2) + kx) << lw; };   // plane row (lw <= 8: one tile per row quad)
+        if (type == 0) {
+          // ---- FAR: a = (ky, kxa) of row quad Y, b = its partner under (x ^ mx, y ^ my); eq. (4) ----------------------
+          const int mx = p1, my = p2;
+          const int ky = phase + 2 * half, kxa = 2 * hi, kyb = ky ^ (my & 3), kxb = kxa ^ (mx & 3), Yb = Y ^ (my >> 2);
+          // b in a's lane order: lane i <-> i ^ c, c = (mx >> 2) & 15: word j of the permuted vector is word j ^ (c >> 2)
+          // of the partner chunk, its bytes permuted by c & 3
+          const int jb = j ^ (((mx >> 2) & 15) >> 2), Xb0 = X0 ^ ((mx >> 2) & Wm & ~15), Xb = Xb0 + 4 * jb;
+          const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
+          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
+          const int kybu = (kyb - 1) & 3, Ybu = (Yb - (kyb == 0)) & Wm, kybd = (kyb + 1) & 3, Ybd = (Yb + (kyb == 3)) & Wm;
+          const int ra = R(ky, kxa, Y), rb = R(kyb, kxb, Yb);
+          A4 = ldw<BITS>(lat, ra, Xj);
+          const uint32_t b0 = ldw<BITS>(lat, rb, Xb);
+          EA4 = ldw_sh<BITS>(lat, R(ky, (kxa + 3) & 3, Y), Xj, W, kxa == 0 ? -1 : 0) + ldw<BITS>(lat, R(ky, kxa + 1, Y), Xj) +
+                ldw<BITS>(lat, R(kyu, kxa, Yu), Xj) + ldw<BITS>(lat, R(kyd, kxa, Yd), Xj);
+          const uint32_t eb0 = ldw<BITS>(lat, R(kyb, kxb - 1, Yb), Xb) + ldw_sh<BITS>(lat, R(kyb, (kxb + 1) & 3, Yb), Xb, W, kxb == 3 ? 1 : 0) +
+                               ldw<BITS>(lat, R(kybu, kxb, Ybu), Xb) + ldw<BITS>(lat, R(kybd, kxb, Ybd), Xb);
+          B4 = __byte_perm(b0, 0u, selb); EB4 = __byte_perm(eb0, 0u, selb);
+          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kxa);
+          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
+          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+          st_word<BITS>(lat, ra, X0, j, A4);
+          st_word<BITS>(lat, rb, Xb0, jb, __byte_perm(B4, 0u, selb));
+          sgn = phase ? -1 : 1;
+          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+          tM += Ma + Mb; tMs += sgn * (Ma + Mb);
+        } else if (p1 == 1) {
+          // ---- NEAR, vertical dominoes: a = (ky, kx), b = the site below; eq. (5) --------------------------------------
+          const int kx = half + 2 * hi, ky = (p2 + 2 * ((half + phase) & 1)) & 3;
+          const int kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
+          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (kyb + 1) & 3, Yd = (Yb + (kyb == 3)) & Wm;
+          const int ra = R(ky, kx, Y), rb = R(kyb, kx, Yb);
+          const int shl = kx == 0 ? -1 : 0, shr = kx == 3 ? 1 : 0;
+          A4 = ldw<BITS>(lat, ra, Xj); B4 = ldw<BITS>(lat, rb, Xj);
+          // vertical domino: a's lower neighbour is b, b's upper neighbour is a
+          EA4 = ldw_sh<BITS>(lat, R(ky, (kx + 3) & 3, Y), Xj, W, shl) + ldw_sh<BITS>(lat, R(ky, (kx + 1) & 3, Y), Xj, W, shr) +
+                ldw<BITS>(lat, R(kyu, kx, Yu), Xj) + B4;
+          EB4 = ldw_sh<BITS>(lat, R(kyb, (kx + 3) & 3, Yb), Xj, W, shl) + ldw_sh<BITS>(lat, R(kyb, (kx + 1) & 3, Yb), Xj, W, shr) +
+                A4 + ldw<BITS>(lat, R(kyd, kx, Yd), Xj);
+          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kx);
+          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
+          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+          st_word<BITS>(lat, ra, X0, j, A4);
+          st_word<BITS>(lat, rb, X0, j, B4);
+          sgn = ((kx + ky) & 1) ? -1 : 1;
+          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+          tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+        } else {
+          // ---- NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site; eq. (5) ------------
+          const int ky = half + 2 * hi;
+          const int ka = (p2 + 2 * ((half + phase) & 1)) & 3, kb = (ka + 1) & 3;
+          const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
+          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
+          const int ra = R(ky, ka, Y), rb = R(ky, kb, Y);
+          A4 = ldw_sh<BITS>(lat, ra, Xj, W, sh_a); B4 = ldw<BITS>(lat, rb, Xj);
+          EA4 = ldw_sh<BITS>(lat, R(ky, (ka + 3) & 3, Y), Xj, W, sh_l) + B4 +
+                ldw_sh<BITS>(lat, R(kyu, ka, Yu), Xj, W, sh_a) + ldw_sh<BITS>(lat, R(kyd, ka, Yd), Xj, W, sh_a);
+          EB4 = A4 + ldw_sh<BITS>(lat, R(ky, (kb + 1) & 3, Y), Xj, W, sh_r) +
+                ldw<BITS>(lat, R(kyu, kb, Yu), Xj) + ldw<BITS>(lat, R(kyd, kb, Yd), Xj);
+          const uint32_t A4old = A4;
+          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kb);
+          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
+          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+          st_word<BITS>(lat, rb, X0, j, B4);
+          if (sh_a == 0) st_word<BITS>(lat, ra, X0, j, A4); else st_word_left1<BITS>(lat, ra, X0, W, j, A4, A4old);
+          sgn = ((ka + ky) & 1) ? -1 : 1;
+          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+          tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+        }
+        // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
+        const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
+        const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
+        tJ += j11; tV += v11; tn2 += a3;
+      }
+      // block sums -> the sweep's accumulator
+      if (phase == 1) {
+        __shared__ int red[5][COOP_THREADS / 32];
+        const unsigned full = 0xFFFFFFFFu;
+        tn2 = __reduce_add_sync(full, tn2); tV = __reduce_add_sync(full, tV); tJ = __reduce_add_sync(full, tJ);
+        tM = __reduce_add_sync(full, tM); tMs = __reduce_add_sync(full, tMs);
+        const int warp = tid >> 5;
+        if (lane == 0) { red[0][warp] = tn2; red[1][warp] = tV; red[2][warp] = tJ; red[3][warp] = tM; red[4][warp] = tMs; }
+        __syncthreads();
+        if (warp == 0) {
+#pragma unroll
+          for (int k = 0; k < 5; ++k) {
+            const int v = __reduce_add_sync(full, lane < COOP_THREADS / 32 ? red[k][lane] : 0);
+            if (lane == 0 && v) atomicAdd((unsigned long long*)&acc[k], (unsigned long long)(long long)v);
+          }
+        }
+      }
+      bar_target += gridDim.x;
+      coop_barrier(&sc->arrived, bar_target);       // phase 1 reads neighbours written in phase 0; the fold reads all sums
+    }
+    if (folder) {
+      volatile long long* va = acc;
+      o.n2 += va[0]; o.bV += va[1]; o.bJ += va[2]; o.M = va[3]; o.Ms = va[4];    // the two phases covered every site once
+      va[0] = 0; va[1] = 0; va[2] = 0; va[3] = 0; va[4] = 0;                     // reused two sweeps (four barriers) from now
+      // U5, one rounding per operation, the order of k_fold
+      const double E = __dadd_rn(__dadd_rn(__dmul_rn(A.delta, (double)o.n2), __dmul_rn(A.V, (double)o.bV)),
+                                 __dmul_rn(A.quarterJ, (double)o.bJ));
+      const double M = (double)o.M, Ms = (double)o.Ms;
+      o.sumE = __dadd_rn(o.sumE, E); o.sumE2 = __dadd_rn(o.sumE2, __dmul_rn(E, E));
+      o.sumM = __dadd_rn(o.sumM, M); o.sumM2 = __dadd_rn(o.sumM2, __dmul_rn(M, M)); o.sumAbsM = __dadd_rn(o.sumAbsM, fabs(M));
+      o.sumMs = __dadd_rn(o.sumMs, Ms); o.sumMs2 = __dadd_rn(o.sumMs2, __dmul_rn(Ms, Ms)); o.sumAbsMs = __dadd_rn(o.sumAbsMs, fabs(Ms));
+      o.nmeas += 1;
+      if (A.trace) {
+        long long* tr = A.trace + 6LL * ((long long)A.replicas * s + r);
+        tr[0] = o.n2; tr[1] = o.bV; tr[2] = o.bJ; tr[3] = o.M; tr[4] = o.Ms; tr[5] = o.Q;
+      }
+    }
+  }
+  if (folder) A.obs[r] = o;
+}
+
+}  // namespace ic

@@ -361,9 +361,12 @@ def test_staged_kernels_one_block_per_replica(pkg):
 # ------------------------------------------------------------------------------------------------ kernel variants
 @pytest.mark.parametrize("L,reps,nsweeps,variant,bits", [(64, 3, 64, 2, 8), (128, 2, 64, 2, 8), (256, 2, 48, 2, 8), (1024, 1, 40, 2, 8),
                                                          (2048, 2, 32, 2, 8), (2048, 2, 48, 3, 8), (4096, 2, 32, 3, 8), (8192, 1, 12, 3, 8),
-                                                         (2048, 2, 64, 3, 2), (4096, 2, 48, 3, 2), (8192, 1, 16, 3, 2)])
+                                                         (2048, 2, 64, 3, 2), (4096, 2, 48, 3, 2), (8192, 1, 16, 3, 2),
+                                                         (128, 3, 64, 5, 8), (128, 2, 64, 5, 2), (256, 2, 64, 5, 2), (512, 1, 48, 5, 8),
+                                                         (1024, 1, 48, 5, 8), (1024, 2, 48, 5, 2)])
 def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant, bits):
-    """Variant 2 (tiled, L <= 2048) and variant 3 (TMA-staged, L >= 2048) against variant 1 (one thread per pair) on the
+    """Variant 2 (tiled, L <= 2048), variant 3 (TMA-staged, L >= 2048) and variant 5 (one cooperative launch for all the
+    sweeps of a call, 128 <= L <= 1024) against variant 1 (one thread per pair) on the
     same device memory layout, sweep by sweep so that many (mx, my) masks, both domino orientations and all four offsets
     are exercised; the reference kernels are themselves compared with the oracle above and (at L <= 256) here."""
     seed = 4242 + L
@@ -388,6 +391,15 @@ def test_tiled_kernels_equal_reference_kernels(pkg, L, reps, nsweeps, variant, b
     if L <= 256:
         lats, _ = oracle_run(codes, 0.3, 1.0, 1.5, seed, Ts, nsweeps)
         check_against_oracle(a, lats, Ts)
+    if variant == 5:
+        # many sweeps inside ONE launch (the barriers between phases and sweeps are what is new), with the per-sweep trace
+        tra = a.sweep_trace(Ts, 40).cpu().numpy(); trb = b.sweep_trace(Ts, 40).cpu().numpy()
+        assert np.array_equal(tra, trb)
+        a.sweep(Ts, 25); a.sweep(Ts, 15); b.sweep(Ts, 40)
+        assert a.observables() == b.observables()
+        for r in range(reps):
+            assert np.array_equal(a.state(r), b.state(r)), r
+            assert list(a.debug_recompute(r)) == [a.observables()[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
     a.close(); b.close()
 
 
