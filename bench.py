@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C5] [--sweeps-per-step S]
 
-A "step" is one pass of the whole hot path over one batch: S sweeps (default 100 = the whole run of BASELINE config 5)
+A "step" is one pass of the whole hot path over one batch: S sweeps (default: the whole run of the config; 100 for BASELINE config 5)
 of the configured lattice, each sweep = two conflict-free phases of N/4 coupled-pair updates (schedule, loads, Philox,
 proposal, dE class, acceptance, write-back, per-sweep observables and their fp64 accumulation).  One process per GPU; with N > 1 every rank runs its own lattice copy (the path shards over replicas,
 PAPER.md:141; no data-path collective) and the value is the aggregate over ranks ("weak").
@@ -194,7 +194,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C5", choices=sorted(ic_inputs.CONFIGS))
-    ap.add_argument("--sweeps-per-step", type=int, default=100)
+    ap.add_argument("--sweeps-per-step", type=int, default=0, help="0 = the sweeps of the config's whole run (C5: 100)")
     ap.add_argument("--bits", type=int, default=0, help="override bits per site (8 or 2)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -204,6 +204,8 @@ def main():
     cfg = dict(ic_inputs.CONFIGS[args.config])
     if args.bits:
         cfg["bits"] = args.bits
+    if args.sweeps_per_step <= 0:
+        args.sweeps_per_step = int(cfg["sweeps"])
     if args.impl == "reference":
         return run_reference(args, cfg)
 

@@ -464,11 +464,14 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   a.lat_stride = c->lat_stride; a.nsweeps = nsweeps; a.sweep0 = c->sweep; a.delta = c->delta; a.V = c->V; a.quarterJ = 0.25 * c->J;
   a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const long long items = c->N / 16;                                   // four pairs per item, N/4 pairs per phase
-  const long long want = (items + COOP_THREADS - 1) / COOP_THREADS, cap = std::max<long long>(1, c->sm_count / c->replicas);
-  dim3 grid((unsigned)std::min(want, cap), (unsigned)c->replicas);
+  // latency-bound: spread the items of a phase over as many SMs as there are, at least four warps per block
+  const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
+  const long long nblk = std::min(cap, (items + 127) / 128);
+  const int threads = (int)std::min<long long>(COOP_THREADS, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
+  dim3 grid((unsigned)nblk, (unsigned)c->replicas);
   IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
   void* args[] = {(void*)&a};
-  IC_CUDA(cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(COOP_THREADS), args, (size_t)COOP_SMEM_BYTES, c->stream));
+  IC_CUDA(cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream));
   c->launches++;
   return IC_OK;
 }

@@ -83,12 +83,10 @@ __device__ __forceinline__ uint32_t ldw_sh(const uint8_t* lat, int row, int X, i
 template <int BITS>
 __device__ __forceinline__ void st_word(uint8_t* lat, int row, int X0, int j, uint32_t w4) {
   if (BITS == 8) { *reinterpret_cast<uint32_t*>(lat + row + X0 + 4 * j) = w4; return; }
-  // only the quad is named in the mask: at L = 128 the two halves of a warp work on different row classes and may be in
-  // different branches (aligned store / store shifted by one site) when they get here
-  const unsigned qm = 0xFu << ((threadIdx.x & 31) & 28);
+  // (the item order keeps the row class uniform in a warp, so every lane of the warp is here)
   uint32_t p = __funnelshift_l(w4, w4, 2 * j);
-  p |= __shfl_xor_sync(qm, p, 1);
-  p |= __shfl_xor_sync(qm, p, 2);
+  p |= __shfl_xor_sync(0xFFFFFFFFu, p, 1);
+  p |= __shfl_xor_sync(0xFFFFFFFFu, p, 2);
   if (j == 0) *reinterpret_cast<uint32_t*>(lat + ((row + X0) >> 2)) = p;
 }
 // the same for a vector that starts one site to the left (sites X0-1+4j .. X0+2+4j, periodic): bytes cross word borders
@@ -117,14 +115,14 @@ template <int BITS>
 __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs A) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ int s_par[4];
-  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
+  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31, nthr = (int)blockDim.x;
   const uint32_t smem0 = smem_u32(smem);
   {
     const uint2* src = A.thr + (long long)r * THR_STRIDE;
     uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
-    for (int k = tid; k < THR_STRIDE; k += COOP_THREADS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+    for (int k = tid; k < THR_STRIDE; k += nthr) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
     uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
-    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += COOP_THREADS) {
+    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += nthr) {
       const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
       const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
       uint2 d = __ldg(&A.desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
@@ -135,6 +133,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
   const int L = A.L, lw = A.logL - 2, W = 1 << lw, Wm = W - 1;
   const int lognch = lw - 4, nch = 1 << lognch;
   const int n_items = (W * 4 * nch) * 4;                           // (Y, half, hi, chunk, word)
+  const int nlo = lognch < 3 ? 3 - lognch : 0;                     // low bits of Y kept below (hi, half): a warp = one row class
   uint8_t* lat = reinterpret_cast<uint8_t*>(A.lattice) + (long long)r * A.lat_stride;
   CoopScratch* sc = &A.scratch[r];
   const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
@@ -160,9 +159,9 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
     int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;       // this thread's sums over both phases of the sweep
     for (int phase = 0; phase < 2; ++phase) {
       const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
-      for (int it = blockIdx.x * COOP_THREADS + tid; it < n_items; it += gridDim.x * COOP_THREADS) {
-        const int j = it & 3, chunk = (it >> 2) & (nch - 1), hi = (it >> (2 + lognch)) & 1, half = (it >> (3 + lognch)) & 1;
-        const int Y = it >> (4 + lognch), X0 = chunk << 4;
+      for (int it = blockIdx.x * nthr + tid; it < n_items; it += gridDim.x * nthr) {
+        const int j = it & 3, chunk = (it >> 2) & (nch - 1), hi = (it >> (2 + lognch + nlo)) & 1, half = (it >> (3 + lognch + nlo)) & 1;
+        const int Y = ((it >> (4 + lognch + nlo)) << nlo) | ((it >> (2 + lognch)) & ((1 << nlo) - 1)), X0 = chunk << 4;
         uint32_t A4, B4, EA4, EB4, c0;
         int a3 = 0, sgn, y;
         const int Xj = X0 + 4 * j;                                      // plane column of the item's first pair
@@ -256,7 +255,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
         if (warp == 0) {
 #pragma unroll
           for (int k = 0; k < 5; ++k) {
-            const int v = __reduce_add_sync(full, lane < COOP_THREADS / 32 ? red[k][lane] : 0);
+            const int v = __reduce_add_sync(full, lane < (nthr >> 5) ? red[k][lane] : 0);
             if (lane == 0 && v) atomicAdd((unsigned long long*)&acc[k], (unsigned long long)(long long)v);
           }
         }
