@@ -148,13 +148,21 @@ int ic_snapshot_ppm(ic_ctx* ctx, int replica, const char* path);
  * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels
  * (8 or 2 bits/site, L >= 2048: tiles staged in shared memory by TMA bulk copies; the default there).
  * 4 = resident kernel (L <= 64, any bits_per_site: one block per replica keeps its lattice in shared memory and
- * runs all sweeps of an ic_sweep call in one launch; the default for L <= 64).
+ * runs all sweeps of an ic_sweep call in one launch, one thread per pair; the default for L < 16).
+ * 6 = resident kernel with four-pair items (16 <= L <= 64, any bits_per_site: the same, with the item code of the staged
+ * kernels on a byte lattice in shared memory; the default there).
  * 5 = one-launch kernel (8 or 2 bits/site, 128 <= L <= 1024, replicas <= number of SMs: one cooperative launch runs
  * all sweeps of an ic_sweep call on the whole GPU, the phases separated by a barrier over the replica's blocks; the
  * default there).
  * IC_ERR_PARAM if the variant cannot run this context's (L, bits_per_site).  All variants produce identical
  * lattices and observables.                                                                           */
 int ic_set_variant(ic_ctx* ctx, int variant);
+
+/* Upper bound on the thread blocks per replica of the persistent kernels (variants 2, 3, 5); 0 = automatic (one block per
+ * SM divided among the replicas).  Results do not depend on it: the tests run the kernels at several bounds (1, 2, 3, ...)
+ * so that every block walks many tasks and ring laps and the task-to-block assignment changes -- the race check this
+ * library can offer where no sanitizer is available.  IC_ERR_PARAM if max_blocks < 0.                */
+int ic_set_max_blocks(ic_ctx* ctx, int max_blocks);
 
 /* Number of kernels launched by this context since ic_create (for bench.py's gpu_launches).         */
 int64_t ic_launch_count(const ic_ctx* ctx);

@@ -45,6 +45,7 @@ EXPORTS = {
     "ic_sweep_count": (C.c_int64, [C.c_void_p]),
     "ic_charge": (C.c_int64, [C.c_void_p]),
     "ic_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
+    "ic_set_max_blocks": (C.c_int, [C.c_void_p, C.c_int]),
     "ic_launch_count": (C.c_int64, [C.c_void_p]),
     "ic_destroy": (C.c_int, [C.c_void_p]),
     "ic_strerror": (C.c_char_p, [C.c_int]),
@@ -191,6 +192,9 @@ class Sim:
 
     def set_variant(self, variant):
         _check(lib.ic_set_variant(self.h, int(variant)), "ic_set_variant")
+
+    def set_max_blocks(self, max_blocks):
+        _check(lib.ic_set_max_blocks(self.h, int(max_blocks)), "ic_set_max_blocks")
 
     @property
     def sweep_count(self):

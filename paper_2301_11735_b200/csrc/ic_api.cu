@@ -39,7 +39,11 @@ struct ic_ctx {
   long long launches;
   int sm_count, device;
   bool coop_supported;
+  int max_blocks;            // ic_set_max_blocks: 0 = automatic
 };
+static long long blocks_cap(const ic_ctx* c, long long automatic) {
+  return c->max_blocks > 0 ? std::min<long long>(automatic, c->max_blocks) : automatic;
+}
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
@@ -276,7 +280,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   ic_ctx* c = new (std::nothrow) ic_ctx();
   if (!c) return IC_ERR_NULL;
   c->L = L; c->logL = 0; while ((1 << c->logL) < L) c->logL++;
-  c->replicas = replicas; c->bits = bits; c->variant = 0;
+  c->replicas = replicas; c->bits = bits; c->variant = 0; c->max_blocks = 0;
   c->layout = bits == 2 ? (L >= 128 ? LAY_P2 : LAY_ROW2) : (L >= 64 ? LAY_P16 : LAY_ROW8);
   c->N = (long long)L * L; c->Q = std::llround(n * (double)c->N);
   c->n = n; c->delta = delta; c->V = V; c->J = J; c->seed = seed; c->sweep = 0;
@@ -412,7 +416,7 @@ static int launch_phase_ref(ic_ctx* c, const PhaseArgs& a) {
 static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
   const long long n_items = c->N / 128;
   const long long nb = (n_items + P16_THREADS - 1) / P16_THREADS;
-  const long long cap = std::max<long long>(1, ((long long)c->sm_count * 6 + c->replicas - 1) / c->replicas);
+  const long long cap = blocks_cap(c, std::max<long long>(1, ((long long)c->sm_count * 6 + c->replicas - 1) / c->replicas));
   dim3 grid((unsigned)std::min(nb, cap), (unsigned)c->replicas);
   if (a.type == 0) {
     a.desc = c->d_desc;
@@ -465,7 +469,7 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const long long items = c->N / 16;                                   // four pairs per item, N/4 pairs per phase
   // latency-bound: spread the items of a phase over as many SMs as there are, at least four warps per block
-  const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
+  const long long cap = blocks_cap(c, std::max<long long>(1, c->sm_count / c->replicas));
   const long long nblk = std::min(cap, (items + 127) / 128);
   const int threads = (int)std::min<long long>(COOP_THREADS, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
   dim3 grid((unsigned)nblk, (unsigned)c->replicas);
@@ -475,11 +479,31 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   c->launches++;
   return IC_OK;
 }
+// small lattices: one block per replica, lattice resident in shared memory, the items of the one-launch kernel
+static bool resvec_ok(const ic_ctx* c) { return c->L >= RESV_MIN_L && c->L <= RESV_MAX_L; }
+template <int LAYG>
+static int launch_resvec(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
+  static bool configured[64] = {};
+  if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
+    IC_CUDA(cudaFuncSetAttribute(k_resvec_sweeps<LAYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESV_SMEM_BYTES));
+    if (c->device >= 0 && c->device < 64) configured[c->device] = true;
+  }
+  CoopArgs a;
+  a.lattice = c->lattice; a.thr = c->d_thr; a.desc32 = c->d_desc32; a.obs = c->d_obs; a.scratch = c->d_coop; a.trace = (long long*)d_trace;
+  a.lat_stride = c->lat_stride; a.nsweeps = nsweeps; a.sweep0 = c->sweep; a.delta = c->delta; a.V = c->V; a.quarterJ = 0.25 * c->J;
+  a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
+  const long long items = c->N / 16;
+  const int threads = (int)std::min<long long>(COOP_THREADS, std::max<long long>(64, (items + 31) / 32 * 32));
+  k_resvec_sweeps<LAYG><<<c->replicas, threads, RESV_SMEM_BYTES, c->stream>>>(a);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
 static bool staged_ok(const ic_ctx* c) { return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= 4 * ST_SEG; }
 static bool tiled_ok(const ic_ctx* c) { return c->layout == LAY_P16 && c->L <= 4 * ST_SEG; }   // one tile per row quad
 static int launch_phase_staged(ic_ctx* c, PhaseArgs a) {
   const long long ntasks = ((long long)(c->L / 4) * (c->L / 4 / ST_SEG)) / 2;
-  const long long cap = std::max<long long>(1, c->sm_count / c->replicas);
+  const long long cap = blocks_cap(c, std::max<long long>(1, c->sm_count / c->replicas));
   dim3 grid((unsigned)std::min(ntasks, cap), (unsigned)c->replicas);
   a.desc32 = c->d_desc32;
   // Philox: the ten round keys and the parts of the first two rounds that are the same for the whole launch (U3)
@@ -534,6 +558,13 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
   { int rc = ensure_thresholds(c, h_T); if (rc != IC_OK) return rc; }
 
   // small lattices: all the sweeps in one launch, one block per replica, lattice resident in shared memory
+  if (resvec_ok(c) && (c->variant == 0 || c->variant == 6)) {
+    int rc = c->layout == LAY_ROW8 ? launch_resvec<LAY_ROW8>(c, nsweeps, d_trace)
+             : c->layout == LAY_ROW2 ? launch_resvec<LAY_ROW2>(c, nsweeps, d_trace) : launch_resvec<LAY_P16>(c, nsweeps, d_trace);
+    if (rc != IC_OK) return rc;
+    c->sweep += (uint64_t)nsweeps;
+    return IC_OK;
+  }
   if (c->L <= RES_MAX_L && (c->variant == 0 || c->variant == 4)) {
     ResidentArgs ra;
     ra.lattice = c->lattice; ra.thr = c->d_thr; ra.obs = c->d_obs; ra.trace = (long long*)d_trace; ra.lat_stride = c->lat_stride;
@@ -759,12 +790,20 @@ extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->lau
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {
   if (!c) return IC_ERR_NULL;
-  if (variant < 0 || variant > 5) return IC_ERR_PARAM;
+  if (variant < 0 || variant > 6) return IC_ERR_PARAM;
+  if (variant == 6 && !resvec_ok(c)) return IC_ERR_PARAM;
   if (variant == 5 && !coop_ok(c)) return IC_ERR_PARAM;
   if (variant == 4 && c->L > RES_MAX_L) return IC_ERR_PARAM;
   if (variant == 2 && !tiled_ok(c)) return IC_ERR_PARAM;
   if (variant == 3 && !staged_ok(c)) return IC_ERR_PARAM;
   c->variant = variant;
+  return IC_OK;
+}
+
+extern "C" int ic_set_max_blocks(ic_ctx* c, int max_blocks) {
+  if (!c) return IC_ERR_NULL;
+  if (max_blocks < 0) return IC_ERR_PARAM;
+  c->max_blocks = max_blocks;
   return IC_OK;
 }
 

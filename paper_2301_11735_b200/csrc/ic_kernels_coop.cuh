@@ -111,6 +111,108 @@ __device__ __forceinline__ void st_word_left1(uint8_t* lat, int row, int X0, int
   if (own) atomicXor(reinterpret_cast<uint32_t*>(lat + ((row + X0) >> 2)), own);
 }
 
+// Item it of a phase -> (word of the plane row, plane selector hi, row class half, row quad Y).  The word index is the lowest
+// field; then as many low bits of Y as it takes to fill a warp, so that (hi, half) -- which decide the branches taken and
+// the shapes of the stores -- are uniform in a warp whenever the lattice is large enough (L >= 128).
+__device__ __forceinline__ void item_coords(int it, int lw, int& wi, int& hi, int& half, int& Y) {
+  const int lgw = lw - 2;                                            // log2(words per plane row)
+  const int nlo = min(lw, lgw < 5 ? 5 - lgw : 0);
+  wi = it & ((1 << lgw) - 1);
+  hi = (it >> (lgw + nlo)) & 1; half = (it >> (lgw + nlo + 1)) & 1;
+  Y = ((it >> (lgw + nlo + 2)) << nlo) | ((it >> lgw) & ((1 << nlo) - 1));
+}
+
+// One item = the four coupled pairs of word wi of a plane row (PAPER.md:64-98 through pairs4, the item code of the
+// staged kernels): loads of the ten words (a, b, eight neighbours), one Philox block, the update, the stores, and the
+// item's contribution to the sweep's sums.  lat: the replica's lattice in LAY_P16 (BITS = 8; global or shared memory) or
+// LAY_P2 (BITS = 2), one tile per row quad (L <= 2048).
+template <int BITS>
+__device__ __forceinline__ void coop_item(uint8_t* lat, int lw, int type, int p1, int p2, int phase, int wi, int hi, int half, int Y,
+                                          uint32_t c2, uint32_t c3, uint32_t key0, uint32_t key1, uint32_t s_desc,
+                                          int& tn2, int& tV, int& tJ, int& tM, int& tMs) {
+  const int W = 1 << lw, Wm = W - 1;
+  const int Xj = 4 * wi, X0 = Xj & ~15, j = wi & 3;                  // plane column of the item's first pair; its 16-site vector; word in it
+  uint32_t A4, B4, EA4, EB4, c0;
+  int a3 = 0, sgn, y;
+  auto R = [lw](int ky, int kx, int Yq) -> int { return ((Yq << 4) + (ky << 2) + kx) << lw; };   // plane row (lw <= 8: one tile per row quad)
+  if (type == 0) {
+    // ---- FAR: a = (ky, kxa) of row quad Y, b = its partner under (x ^ mx, y ^ my); eq. (4) ----------------------
+    const int mx = p1, my = p2;
+    const int ky = phase + 2 * half, kxa = 2 * hi, kyb = ky ^ (my & 3), kxb = kxa ^ (mx & 3), Yb = Y ^ (my >> 2);
+    // b in a's lane order: lane i <-> i ^ c, c = (mx >> 2) & 15: word j of the permuted vector is word j ^ (c >> 2)
+    // of the partner chunk, its bytes permuted by c & 3
+    const int jb = j ^ (((mx >> 2) & 15) >> 2), Xb0 = X0 ^ ((mx >> 2) & Wm & ~15), Xb = Xb0 + 4 * jb;
+    const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
+    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
+    const int kybu = (kyb - 1) & 3, Ybu = (Yb - (kyb == 0)) & Wm, kybd = (kyb + 1) & 3, Ybd = (Yb + (kyb == 3)) & Wm;
+    const int ra = R(ky, kxa, Y), rb = R(kyb, kxb, Yb);
+    A4 = ldw<BITS>(lat, ra, Xj);
+    const uint32_t b0 = ldw<BITS>(lat, rb, Xb);
+    EA4 = ldw_sh<BITS>(lat, R(ky, (kxa + 3) & 3, Y), Xj, W, kxa == 0 ? -1 : 0) + ldw<BITS>(lat, R(ky, kxa + 1, Y), Xj) +
+          ldw<BITS>(lat, R(kyu, kxa, Yu), Xj) + ldw<BITS>(lat, R(kyd, kxa, Yd), Xj);
+    const uint32_t eb0 = ldw<BITS>(lat, R(kyb, kxb - 1, Yb), Xb) + ldw_sh<BITS>(lat, R(kyb, (kxb + 1) & 3, Yb), Xb, W, kxb == 3 ? 1 : 0) +
+                         ldw<BITS>(lat, R(kybu, kxb, Ybu), Xb) + ldw<BITS>(lat, R(kybd, kxb, Ybd), Xb);
+    B4 = __byte_perm(b0, 0u, selb); EB4 = __byte_perm(eb0, 0u, selb);
+    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kxa);
+    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+    st_word<BITS>(lat, ra, X0, j, A4);
+    st_word<BITS>(lat, rb, Xb0, jb, __byte_perm(B4, 0u, selb));
+    sgn = phase ? -1 : 1;
+    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+    tM += Ma + Mb; tMs += sgn * (Ma + Mb);
+  } else if (p1 == 1) {
+    // ---- NEAR, vertical dominoes: a = (ky, kx), b = the site below; eq. (5) --------------------------------------
+    const int kx = half + 2 * hi, ky = (p2 + 2 * ((half + phase) & 1)) & 3;
+    const int kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
+    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (kyb + 1) & 3, Yd = (Yb + (kyb == 3)) & Wm;
+    const int ra = R(ky, kx, Y), rb = R(kyb, kx, Yb);
+    const int shl = kx == 0 ? -1 : 0, shr = kx == 3 ? 1 : 0;
+    A4 = ldw<BITS>(lat, ra, Xj); B4 = ldw<BITS>(lat, rb, Xj);
+    // vertical domino: a's lower neighbour is b, b's upper neighbour is a
+    EA4 = ldw_sh<BITS>(lat, R(ky, (kx + 3) & 3, Y), Xj, W, shl) + ldw_sh<BITS>(lat, R(ky, (kx + 1) & 3, Y), Xj, W, shr) +
+          ldw<BITS>(lat, R(kyu, kx, Yu), Xj) + B4;
+    EB4 = ldw_sh<BITS>(lat, R(kyb, (kx + 3) & 3, Yb), Xj, W, shl) + ldw_sh<BITS>(lat, R(kyb, (kx + 1) & 3, Yb), Xj, W, shr) +
+          A4 + ldw<BITS>(lat, R(kyd, kx, Yd), Xj);
+    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kx);
+    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+    st_word<BITS>(lat, ra, X0, j, A4);
+    st_word<BITS>(lat, rb, X0, j, B4);
+    sgn = ((kx + ky) & 1) ? -1 : 1;
+    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+    tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+  } else {
+    // ---- NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site; eq. (5) ------------
+    const int ky = half + 2 * hi;
+    const int ka = (p2 + 2 * ((half + phase) & 1)) & 3, kb = (ka + 1) & 3;
+    const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
+    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
+    const int ra = R(ky, ka, Y), rb = R(ky, kb, Y);
+    A4 = ldw_sh<BITS>(lat, ra, Xj, W, sh_a); B4 = ldw<BITS>(lat, rb, Xj);
+    EA4 = ldw_sh<BITS>(lat, R(ky, (ka + 3) & 3, Y), Xj, W, sh_l) + B4 +
+          ldw_sh<BITS>(lat, R(kyu, ka, Yu), Xj, W, sh_a) + ldw_sh<BITS>(lat, R(kyd, ka, Yd), Xj, W, sh_a);
+    EB4 = A4 + ldw_sh<BITS>(lat, R(ky, (kb + 1) & 3, Y), Xj, W, sh_r) +
+          ldw<BITS>(lat, R(kyu, kb, Yu), Xj) + ldw<BITS>(lat, R(kyd, kb, Yd), Xj);
+    const uint32_t A4old = A4;
+    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kb);
+    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
+    st_word<BITS>(lat, rb, X0, j, B4);
+    if (sh_a == 0) st_word<BITS>(lat, ra, X0, j, A4); else st_word_left1<BITS>(lat, ra, X0, W, j, A4, A4old);
+    sgn = ((ka + ky) & 1) ? -1 : 1;
+    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
+    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+    tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+  }
+  // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
+  const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
+  const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
+  tJ += j11; tV += v11; tn2 += a3;
+}
+
 template <int BITS>
 __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs A) {
   extern __shared__ __align__(128) unsigned char smem[];
@@ -130,10 +232,8 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
       desc_s[k] = d;
     }
   }
-  const int L = A.L, lw = A.logL - 2, W = 1 << lw, Wm = W - 1;
-  const int lognch = lw - 4, nch = 1 << lognch;
-  const int n_items = (W * 4 * nch) * 4;                           // (Y, half, hi, chunk, word)
-  const int nlo = lognch < 3 ? 3 - lognch : 0;                     // low bits of Y kept below (hi, half): a warp = one row class
+  const int L = A.L, lw = A.logL - 2;
+  const int n_items = 1 << (2 * lw);                               // (row quad, half, hi, word of the plane row): N/16 items of 4 pairs
   uint8_t* lat = reinterpret_cast<uint8_t*>(A.lattice) + (long long)r * A.lat_stride;
   CoopScratch* sc = &A.scratch[r];
   const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
@@ -160,88 +260,9 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
     for (int phase = 0; phase < 2; ++phase) {
       const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
       for (int it = blockIdx.x * nthr + tid; it < n_items; it += gridDim.x * nthr) {
-        const int j = it & 3, chunk = (it >> 2) & (nch - 1), hi = (it >> (2 + lognch + nlo)) & 1, half = (it >> (3 + lognch + nlo)) & 1;
-        const int Y = ((it >> (4 + lognch + nlo)) << nlo) | ((it >> (2 + lognch)) & ((1 << nlo) - 1)), X0 = chunk << 4;
-        uint32_t A4, B4, EA4, EB4, c0;
-        int a3 = 0, sgn, y;
-        const int Xj = X0 + 4 * j;                                      // plane column of the item's first pair
-        auto R = [lw](int ky, int kx, int Yq) -> int { return ((Yq << 4) + (ky << 2) + kx) << lw; };   // plane row (lw <= 8: one tile per row quad)
-        if (type == 0) {
-          // ---- FAR: a = (ky, kxa) of row quad Y, b = its partner under (x ^ mx, y ^ my); eq. (4) ----------------------
-          const int mx = p1, my = p2;
-          const int ky = phase + 2 * half, kxa = 2 * hi, kyb = ky ^ (my & 3), kxb = kxa ^ (mx & 3), Yb = Y ^ (my >> 2);
-          // b in a's lane order: lane i <-> i ^ c, c = (mx >> 2) & 15: word j of the permuted vector is word j ^ (c >> 2)
-          // of the partner chunk, its bytes permuted by c & 3
-          const int jb = j ^ (((mx >> 2) & 15) >> 2), Xb0 = X0 ^ ((mx >> 2) & Wm & ~15), Xb = Xb0 + 4 * jb;
-          const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
-          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
-          const int kybu = (kyb - 1) & 3, Ybu = (Yb - (kyb == 0)) & Wm, kybd = (kyb + 1) & 3, Ybd = (Yb + (kyb == 3)) & Wm;
-          const int ra = R(ky, kxa, Y), rb = R(kyb, kxb, Yb);
-          A4 = ldw<BITS>(lat, ra, Xj);
-          const uint32_t b0 = ldw<BITS>(lat, rb, Xb);
-          EA4 = ldw_sh<BITS>(lat, R(ky, (kxa + 3) & 3, Y), Xj, W, kxa == 0 ? -1 : 0) + ldw<BITS>(lat, R(ky, kxa + 1, Y), Xj) +
-                ldw<BITS>(lat, R(kyu, kxa, Yu), Xj) + ldw<BITS>(lat, R(kyd, kxa, Yd), Xj);
-          const uint32_t eb0 = ldw<BITS>(lat, R(kyb, kxb - 1, Yb), Xb) + ldw_sh<BITS>(lat, R(kyb, (kxb + 1) & 3, Yb), Xb, W, kxb == 3 ? 1 : 0) +
-                               ldw<BITS>(lat, R(kybu, kxb, Ybu), Xb) + ldw<BITS>(lat, R(kybd, kxb, Ybd), Xb);
-          B4 = __byte_perm(b0, 0u, selb); EB4 = __byte_perm(eb0, 0u, selb);
-          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kxa);
-          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
-          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
-          st_word<BITS>(lat, ra, X0, j, A4);
-          st_word<BITS>(lat, rb, Xb0, jb, __byte_perm(B4, 0u, selb));
-          sgn = phase ? -1 : 1;
-          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-          tM += Ma + Mb; tMs += sgn * (Ma + Mb);
-        } else if (p1 == 1) {
-          // ---- NEAR, vertical dominoes: a = (ky, kx), b = the site below; eq. (5) --------------------------------------
-          const int kx = half + 2 * hi, ky = (p2 + 2 * ((half + phase) & 1)) & 3;
-          const int kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (kyb + 1) & 3, Yd = (Yb + (kyb == 3)) & Wm;
-          const int ra = R(ky, kx, Y), rb = R(kyb, kx, Yb);
-          const int shl = kx == 0 ? -1 : 0, shr = kx == 3 ? 1 : 0;
-          A4 = ldw<BITS>(lat, ra, Xj); B4 = ldw<BITS>(lat, rb, Xj);
-          // vertical domino: a's lower neighbour is b, b's upper neighbour is a
-          EA4 = ldw_sh<BITS>(lat, R(ky, (kx + 3) & 3, Y), Xj, W, shl) + ldw_sh<BITS>(lat, R(ky, (kx + 1) & 3, Y), Xj, W, shr) +
-                ldw<BITS>(lat, R(kyu, kx, Yu), Xj) + B4;
-          EB4 = ldw_sh<BITS>(lat, R(kyb, (kx + 3) & 3, Yb), Xj, W, shl) + ldw_sh<BITS>(lat, R(kyb, (kx + 1) & 3, Yb), Xj, W, shr) +
-                A4 + ldw<BITS>(lat, R(kyd, kx, Yd), Xj);
-          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kx);
-          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
-          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
-          st_word<BITS>(lat, ra, X0, j, A4);
-          st_word<BITS>(lat, rb, X0, j, B4);
-          sgn = ((kx + ky) & 1) ? -1 : 1;
-          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-          tM += Ma + Mb; tMs += sgn * (Ma - Mb);
-        } else {
-          // ---- NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site; eq. (5) ------------
-          const int ky = half + 2 * hi;
-          const int ka = (p2 + 2 * ((half + phase) & 1)) & 3, kb = (ka + 1) & 3;
-          const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
-          const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
-          const int ra = R(ky, ka, Y), rb = R(ky, kb, Y);
-          A4 = ldw_sh<BITS>(lat, ra, Xj, W, sh_a); B4 = ldw<BITS>(lat, rb, Xj);
-          EA4 = ldw_sh<BITS>(lat, R(ky, (ka + 3) & 3, Y), Xj, W, sh_l) + B4 +
-                ldw_sh<BITS>(lat, R(kyu, ka, Yu), Xj, W, sh_a) + ldw_sh<BITS>(lat, R(kyd, ka, Yd), Xj, W, sh_a);
-          EB4 = A4 + ldw_sh<BITS>(lat, R(ky, (kb + 1) & 3, Y), Xj, W, sh_r) +
-                ldw<BITS>(lat, R(kyu, kb, Yu), Xj) + ldw<BITS>(lat, R(kyd, kb, Yd), Xj);
-          const uint32_t A4old = A4;
-          y = 4 * Y + ky; c0 = (uint32_t)(4 * (4 * chunk + j) + kb);
-          const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, A.key0, A.key1);
-          pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
-          st_word<BITS>(lat, rb, X0, j, B4);
-          if (sh_a == 0) st_word<BITS>(lat, ra, X0, j, A4); else st_word_left1<BITS>(lat, ra, X0, W, j, A4, A4old);
-          sgn = ((ka + ky) & 1) ? -1 : 1;
-          const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-          const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-          tM += Ma + Mb; tMs += sgn * (Ma - Mb);
-        }
-        // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
-        const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
-        const int v11 = (a3 << 21) >> 21; a3 = (a3 - v11) >> 11;
-        tJ += j11; tV += v11; tn2 += a3;
+        int wi, hi, half, Y;
+        item_coords(it, lw, wi, hi, half, Y);
+        coop_item<BITS>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
       }
       // block sums -> the sweep's accumulator
       if (phase == 1) {
@@ -282,6 +303,113 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
     }
   }
   if (folder) A.obs[r] = o;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Small lattices (16 <= L <= 64, configs C1 and C2): the same items with the replica's lattice resident in shared memory.
+// One block per replica runs all the sweeps of an ic_sweep call; the lattice is converted from its layout in global memory
+// (LAYG: ROW8, ROW2 or P16) to P16 bytes on the way in and back on the way out, the phases are separated by
+// __syncthreads, thread 0 folds the sweep (U5).
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int RESV_MIN_L = 16, RESV_MAX_L = 64;
+constexpr int RESV_OFF_LAT = COOP_SMEM_BYTES;
+constexpr int RESV_SMEM_BYTES = RESV_OFF_LAT + RESV_MAX_L * RESV_MAX_L;
+
+template <int LAYG>
+__global__ void __launch_bounds__(COOP_THREADS, 1) k_resvec_sweeps(const CoopArgs A) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ int s_par[4];
+  __shared__ int red[5][COOP_THREADS / 32];
+  const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, nthr = (int)blockDim.x;
+  const uint32_t smem0 = smem_u32(smem);
+  const int L = A.L, logL = A.logL, lw = logL - 2, N = L * L;
+  const LatView gv{(char*)A.lattice + (long long)r * A.lat_stride, L, logL};
+  uint8_t* lat = smem + RESV_OFF_LAT;
+  {
+    const uint2* src = A.thr + (long long)r * THR_STRIDE;
+    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
+    for (int k = tid; k < THR_STRIDE; k += nthr) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+    uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
+    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += nthr) {
+      const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
+      const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
+      uint2 d = __ldg(&A.desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
+      d.y += smem0 + COOP_OFF_THR;
+      desc_s[k] = d;
+    }
+    for (int i = tid; i < N; i += nthr) {
+      const int x = i & (L - 1), y = i >> logL;
+      lat[p16_site(lw, x, y)] = (uint8_t)e_of_code(Sites<LAYG>::load(gv, x, y));
+    }
+  }
+  const int n_items = 1 << (2 * lw);
+  const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
+  ReplicaObs o;
+  if (tid == 0) o = A.obs[r];
+  __syncthreads();
+
+  for (long long s = 0; s < A.nsweeps; ++s) {
+    const unsigned long long sweep = A.sweep0 + (unsigned long long)s;
+    if (tid == 0) {
+      // U4: parameters of the sweep, the same for all replicas (identical maps for all copies)
+      const u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, A.key0, A.key1);
+      if ((sweep & 1) == 0) { s_par[0] = 0; s_par[1] = (int)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); s_par[2] = (int)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1); }
+      else { s_par[0] = 1; s_par[1] = (int)(z.v[0] & 1u); s_par[2] = (int)(z.v[1] & 3u); }
+    }
+    __syncthreads();
+    const int type = s_par[0], p1 = s_par[1], p2 = s_par[2];
+    const uint32_t s_desc = smem0 + COOP_OFF_DESC + (type ? ST_DESC_SMEM : 0) + (uint32_t)(lane & 15) * 8u;
+    int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
+    for (int phase = 0; phase < 2; ++phase) {
+      const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
+      for (int it = tid; it < n_items; it += nthr) {
+        int wi, hi, half, Y;
+        item_coords(it, lw, wi, hi, half, Y);
+        coop_item<8>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
+      }
+      __syncthreads();       // phase 1 reads neighbours written in phase 0
+    }
+    const unsigned full = 0xFFFFFFFFu;
+    tn2 = __reduce_add_sync(full, tn2); tV = __reduce_add_sync(full, tV); tJ = __reduce_add_sync(full, tJ);
+    tM = __reduce_add_sync(full, tM); tMs = __reduce_add_sync(full, tMs);
+    if (lane == 0) { const int warp = tid >> 5; red[0][warp] = tn2; red[1][warp] = tV; red[2][warp] = tJ; red[3][warp] = tM; red[4][warp] = tMs; }
+    __syncthreads();
+    if (tid == 0) {
+      long long M = 0, Ms = 0;
+      for (int wv = 0; wv < (nthr >> 5); ++wv) { o.n2 += red[0][wv]; o.bV += red[1][wv]; o.bJ += red[2][wv]; M += red[3][wv]; Ms += red[4][wv]; }
+      o.M = M; o.Ms = Ms;                                  // the two phases covered every site once
+      // U5, one rounding per operation, the order of k_fold
+      const double E = __dadd_rn(__dadd_rn(__dmul_rn(A.delta, (double)o.n2), __dmul_rn(A.V, (double)o.bV)),
+                                 __dmul_rn(A.quarterJ, (double)o.bJ));
+      const double Md = (double)o.M, Msd = (double)o.Ms;
+      o.sumE = __dadd_rn(o.sumE, E); o.sumE2 = __dadd_rn(o.sumE2, __dmul_rn(E, E));
+      o.sumM = __dadd_rn(o.sumM, Md); o.sumM2 = __dadd_rn(o.sumM2, __dmul_rn(Md, Md)); o.sumAbsM = __dadd_rn(o.sumAbsM, fabs(Md));
+      o.sumMs = __dadd_rn(o.sumMs, Msd); o.sumMs2 = __dadd_rn(o.sumMs2, __dmul_rn(Msd, Msd)); o.sumAbsMs = __dadd_rn(o.sumAbsMs, fabs(Msd));
+      o.nmeas += 1;
+      if (A.trace) {
+        long long* tr = A.trace + 6LL * ((long long)A.replicas * s + r);
+        tr[0] = o.n2; tr[1] = o.bV; tr[2] = o.bJ; tr[3] = o.M; tr[4] = o.Ms; tr[5] = o.Q;
+      }
+    }
+    // red is rewritten only after the three barriers of the next sweep
+  }
+  __syncthreads();
+  // the lattice goes back in its layout
+  if (LAYG == LAY_ROW2) {
+    uint32_t* words = reinterpret_cast<uint32_t*>(gv.base);
+    for (int wi = tid; wi < (N >> 4); wi += nthr) {
+      uint32_t wd = 0;
+      const int y = (16 * wi) >> logL, x0 = (16 * wi) & (L - 1);
+#pragma unroll
+      for (int k = 0; k < 16; ++k) wd |= (uint32_t)code_of_e(lat[p16_site(lw, x0 + k, y)]) << (2 * k);
+      words[wi] = wd;
+    }
+  } else if (LAYG == LAY_ROW8) {
+    for (int i = tid; i < N; i += nthr) ((int8_t*)gv.base)[i] = (int8_t)code_of_e(lat[p16_site(lw, i & (L - 1), i >> logL)]);
+  } else {
+    for (int i = tid; i < N; i += nthr) ((uint8_t*)gv.base)[i] = lat[i];
+  }
+  if (tid == 0) A.obs[r] = o;
 }
 
 }  // namespace ic

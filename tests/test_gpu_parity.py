@@ -441,17 +441,40 @@ def test_staged_kernels_self_partnered_regions(pkg):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("L,bits,reps", [(4, 8, 2), (8, 2, 3), (16, 8, 5), (32, 2, 2), (64, 8, 3), (64, 2, 2)])
-def test_resident_kernel_equals_reference_kernels(pkg, L, bits, reps):
-    """Variant 4 (one launch for all sweeps, lattice resident in shared memory; the default for L <= 64) against variant 1
-    (one thread per pair, three launches per sweep): lattices, integers, fp64 sums and the per-sweep trace, with the call
-    split in two on one side and a temperature change in between."""
+@pytest.mark.parametrize("L,bits,variant", [(2048, 8, 3), (2048, 2, 3), (4096, 8, 3), (512, 8, 5), (512, 2, 5), (1024, 8, 2)])
+def test_results_do_not_depend_on_the_number_of_blocks(pkg, L, bits, variant):
+    """The persistent kernels with 1, 2, 3, 5, 37 blocks per replica and with the automatic grid: every block then walks
+    many tasks (many laps of the staged kernels' shared-memory ring, many arrivals at the one-launch kernel's barrier) and
+    the task-to-block assignment changes.  Lattices and observables must equal those of the one-thread-per-pair kernels
+    after every sweep group.  (No sanitizer is available on the GPU pool; this is the race check the library offers.)"""
+    seed, nsw = 555 + L, 12
+    nplus, nminus = L * L // 10, L * L // 25
+    code = ic_inputs.random_state(L, nplus, nminus, seed)
+    ref = pkg.Sim(L, (nplus - nminus) / (L * L), 0.3, 1.0, 1.5, seed=seed, bits_per_site=bits); ref.set_variant(1); ref.set_state(0, code)
+    ref.sweep(0.9, nsw)
+    want, wobs = ref.state(0).copy(), ref.observables()[0]
+    ref.close()
+    for cap in (1, 2, 3, 5, 37, 0):
+        sim = pkg.Sim(L, (nplus - nminus) / (L * L), 0.3, 1.0, 1.5, seed=seed, bits_per_site=bits)
+        sim.set_variant(variant); sim.set_max_blocks(cap); sim.set_state(0, code)
+        sim.sweep(0.9, nsw // 2); sim.sweep(0.9, nsw - nsw // 2)
+        assert np.array_equal(sim.state(0), want), cap
+        assert sim.observables()[0] == wobs, cap
+        sim.close()
+
+
+@pytest.mark.parametrize("L,bits,reps,variant", [(4, 8, 2, 4), (8, 2, 3, 4), (16, 8, 5, 4), (32, 2, 2, 4), (64, 8, 3, 4), (64, 2, 2, 4),
+                                                 (16, 8, 5, 6), (16, 2, 3, 6), (32, 8, 2, 6), (32, 2, 2, 6), (64, 8, 3, 6), (64, 2, 2, 6)])
+def test_resident_kernel_equals_reference_kernels(pkg, L, bits, reps, variant):
+    """Variants 4 and 6 (one launch for all sweeps, lattice resident in shared memory: one thread per pair / four-pair items,
+    the defaults for L < 16 / 16 <= L <= 64) against variant 1 (one thread per pair, three launches per sweep): lattices,
+    integers, fp64 sums and the per-sweep trace, with the call split in two on one side and a temperature change in between."""
     seed = 900 + L + bits
     nplus, nminus = L * L // 8, L * L // 16
     n = (nplus - nminus) / (L * L)
     Ts = [0.3, 0.9, 1.7, 2.6, 3.9][:reps]
     codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
-    a = pkg.Sim(L, n, -0.5, 1.0, 2.0, seed=seed, replicas=reps, bits_per_site=bits); a.set_variant(4)
+    a = pkg.Sim(L, n, -0.5, 1.0, 2.0, seed=seed, replicas=reps, bits_per_site=bits); a.set_variant(variant)
     b = pkg.Sim(L, n, -0.5, 1.0, 2.0, seed=seed, replicas=reps, bits_per_site=bits); b.set_variant(1)
     for r in range(reps):
         a.set_state(r, codes[r]); b.set_state(r, codes[r])
