@@ -1,10 +1,11 @@
 // ic_kernels_p16.cuh -- variant 2: the tiled sm_100a kernels on the tiled layout LAY_P16 for 64 <= L <= 2048 (one tile
 // per row quad: a plane row is a whole lattice row), vectors loaded straight from global memory.  Also the home of the
-// 16-byte vector helpers and the layout converters that the staged kernels (ic_kernels_staged.cuh) share.
+// 16-byte vector helpers (with the widen / pack of the 2-bit layout LAY_P2) and the layout converters that the staged and
+// one-launch kernels (ic_kernels_staged.cuh, ic_kernels_coop.cuh) share.
 //
 // One phase of a sweep = one launch.  In every phase of schedule S1 the a-sites and the b-sites are whole plane rows
 // [y&3][x&3] of the layout, so a thread works on dense 16-byte vectors: an "item" is two vectors of 16 coupled pairs
-// (32 pair updates), eight Philox4x32-10 blocks.  Per item:
+// (32 pair updates), eight Philox4x32-7 blocks.  Per item:
 //   1. 128-bit loads of the a- and b-vectors and of their neighbour vectors (A2 of SURVEY 8(a)); the neighbour sums
 //      of 4 sites are byte-wise 32-bit adds: byte = F | G<<3, sum S = F+G-4, sum sigma = F-G;
 //   2. per 4 pairs: a 4x4 byte transpose gives W_i = (8Fa, 8Ga, 8Fb, 8Gb); the pair key (fa,fb,ga,gb) and the

@@ -1,4 +1,6 @@
-// ic_kernels_staged.cuh -- variant 3: the production sm_100a kernels for L >= 2048 on the tiled layout LAY_P16.
+// ic_kernels_staged.cuh -- variant 3: the production sm_100a kernels for L >= 2048 on the tiled layouts LAY_P16 (one byte per
+// site, BITS = 8) and LAY_P2 (two bits per site, BITS = 2: the same tiles with 16 plane sites per 32-bit word; bulk copies move
+// the packed regions, consumers widen a word to the 16-byte vector on load and pack on store).
 //
 // One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM, launched as a programmatic
 // dependent of the previous kernel of the stream (table fill and barrier set-up overlap that kernel's tail):
