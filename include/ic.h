@@ -8,8 +8,11 @@
  * validates arguments, builds the acceptance-threshold tables and the O(1) schedule parameters, and launches.
  *
  * Conventions
- *   - plain C, no exceptions; every entry point returns IC_OK (0) or a negative IC_ERR_* code and leaves
- *     the context unchanged on error.  ic_strerror() gives the text (for IC_ERR_CUDA the CUDA message).
+ *   - plain C, no exceptions; every entry point returns IC_OK (0) or a negative IC_ERR_* code.  Argument errors
+ *     (NULL, SIZE, PARAM, WORKSPACE, CHARGE) are detected before anything is touched and leave the context
+ *     unchanged.  After IC_ERR_CUDA (a launch or copy failed mid-call) the lattices and the sweep counter are
+ *     undefined: the context is only good for ic_destroy.  ic_strerror() gives the text (for IC_ERR_CUDA the
+ *     CUDA message).
  *   - pointers named h_* are HOST memory, d_* are DEVICE memory; both stay owned by the caller.  The
  *     library never allocates device memory: everything it keeps on the device lives inside the
  *     caller-provided workspace (a torch tensor in the Python binding).
@@ -21,7 +24,9 @@
  *     E = Delta*n2 + V*bV + (J/4)*bJ;  M = sum sigma_i, Ms = sum (-1)^(x+y) sigma_i, Q = sum S_i.
  *   - the constraint of eq. (2), sum_i S_i = Q = llround(n*N), holds after every pair update.
  *   - all launches and copies go to the CUDA stream given to ic_create.  ic_sweep is asynchronous;
- *     ic_observables, ic_state, ic_debug_recompute and ic_thresholds synchronise that stream.
+ *     ic_set_state, ic_init_charges, ic_observables, ic_state, ic_debug_recompute, ic_largest_cluster and
+ *     ic_snapshot_ppm synchronise that stream (ic_thresholds and ic_schedule are host-only).  Every call makes the
+ *     device the context was created on current for the calling thread (and leaves it current).
  *   - one context must not be used from two host threads at once.
  */
 #ifndef IC_H

@@ -125,7 +125,8 @@ class Sim:
     def sweep_trace(self, T, nsweeps):
         """Returns a device int64 tensor [nsweeps, replicas, 6] = (n2, bV, bJ, M, Ms, Q) after every sweep."""
         arr, p = self._T(T)
-        tr = self.torch.empty((int(nsweeps), self.replicas, 6), dtype=self.torch.int64, device=self.device)
+        with self.torch.cuda.device(self.device), self.torch.cuda.stream(self.stream):      # the stream ic_create was given
+            tr = self.torch.empty((int(nsweeps), self.replicas, 6), dtype=self.torch.int64, device=self.device)
         _check(lib.ic_sweep_trace(self.h, p, int(nsweeps), C.c_void_p(tr.data_ptr())), "ic_sweep_trace")
         return tr
 

@@ -57,6 +57,13 @@ static int cuda_fail(cudaError_t e, const char* what) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call);      \
   } while (0)
 
+// every entry point that touches the device first makes the context's device current (a caller may have switched)
+#define IC_ENTER(c)                                                                \
+  do {                                                                             \
+    int dev_ = -1;                                                                 \
+    if (cudaGetDevice(&dev_) != cudaSuccess || dev_ != (c)->device) IC_CUDA(cudaSetDevice((c)->device)); \
+  } while (0)
+
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 static bool valid_dims(int L, int replicas, int bits) {
   return L >= 4 && L <= 65536 && (L & (L - 1)) == 0 && replicas >= 1 && replicas <= 65535 && (bits == 8 || bits == 2);
@@ -114,12 +121,13 @@ static void build_class_table(const ic_ctx* c, double T, uint2* out) {
 //   y = 8*K | (xor of the site bytes: a at bits 0,3, b at bits 1,4) << 16 | (dM & 15 | (dD & 15) << 4) << 24,
 //       K = class_index(E_Delta, adj*dS_a*dS_b, adj*dsig_a*dsig_b)  (eq. 4 for adj = 0, eq. 5 for adj = 1),
 //       dM = dsig_a + dsig_b, dD = dsig_a - dsig_b.
-// Null proposals (q = +-2, r >= 6 for q = 0, the current configuration) have x = 0 and no change: class (0,0,0).
+// Null proposals (q = +-2, r >= 6 for q = 0, the current configuration) have x = 0, no change and the class entry
+// NULL_CLASS (threshold 0: never "accepted", see ic_common.cuh).
 static void build_descriptors(int adj, uint2* out) {
   static const int Q0[6][2] = {{2, 3}, {3, 2}, {0, 0}, {1, 1}, {0, 1}, {1, 0}};
   for (int key = 0; key < 28; ++key)
     for (int r = 0; r < 8; ++r) {
-      uint2 d; d.x = 0u; d.y = 8u * (uint32_t)class_index(0, 0, 0);
+      uint2 d; d.x = 0u; d.y = 8u * (uint32_t)NULL_CLASS;
       const int ea = (key & 1) | (key & 8), eb = ((key >> 1) & 1) | ((key >> 1) & 8);
       const bool valid = (key & ~0x1B) == 0;
       if (valid) {
@@ -155,7 +163,7 @@ static void build_descriptors32(uint2* out) {
   for (int adj = 0; adj < 2; ++adj) {
     build_descriptors(adj, d8.data());
     for (int e = 0; e < ST_DESC_ENTRIES; ++e) {
-      uint2 q; q.x = 0u; q.y = 4u * (uint32_t)class_index(0, 0, 0);
+      uint2 q; q.x = 0u; q.y = 4u * (uint32_t)NULL_CLASS;
       if (e < DESC_ENTRIES) {
         const uint2 d = d8[e];
         // the kernel feeds (4F, 8G) per site: halve the G coefficients (CLS_SB dS - dsig is even: CLS_SB is odd)
@@ -352,6 +360,7 @@ extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nm
   if (!c) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
   if (nplus < 0 || nminus < 0 || nplus + nminus > c->N || nplus - nminus != c->Q) return IC_ERR_CHARGE;
+  IC_ENTER(c);
   std::vector<int8_t> codes((size_t)c->N);
   stage1_init(codes.data(), c->N, nplus, nminus, c->seed, replica);
   int rc = upload_state(c, replica, codes.data(), false);
@@ -363,6 +372,7 @@ extern "C" int ic_init_charges(ic_ctx* c, int replica, int64_t nplus, int64_t nm
 extern "C" int ic_set_state(ic_ctx* c, int replica, const int8_t* h_codes) {
   if (!c || !h_codes) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  IC_ENTER(c);
   int rc = upload_state(c, replica, h_codes, true);
   if (rc != IC_OK) return rc;
   IC_CUDA(cudaStreamSynchronize(c->stream));   // h_codes may be pageable and is the caller's to reuse
@@ -372,6 +382,7 @@ extern "C" int ic_set_state(ic_ctx* c, int replica, const int8_t* h_codes) {
 extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
   if (!c || !h_out) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  IC_ENTER(c);
   const char* lat = c->lattice + (long long)replica * c->lat_stride;
   if (c->layout == LAY_ROW8) {
     IC_CUDA(cudaMemcpyAsync(h_out, lat, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
@@ -555,6 +566,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
   if (nsweeps == 0) return IC_OK;
 
+  IC_ENTER(c);
   { int rc = ensure_thresholds(c, h_T); if (rc != IC_OK) return rc; }
 
   // small lattices: all the sweeps in one launch, one block per replica, lattice resident in shared memory
@@ -631,6 +643,7 @@ __global__ void k_reset_sums(ReplicaObs* obs, int replicas) {
 
 extern "C" int ic_reset_observables(ic_ctx* c) {
   if (!c) return IC_ERR_NULL;
+  IC_ENTER(c);
   k_reset_sums<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas);
   c->launches++;
   IC_CUDA(cudaGetLastError());
@@ -639,6 +652,7 @@ extern "C" int ic_reset_observables(ic_ctx* c) {
 
 extern "C" int ic_observables(ic_ctx* c, ic_obs* h_out) {
   if (!c || !h_out) return IC_ERR_NULL;
+  IC_ENTER(c);
   IC_CUDA(cudaMemcpyAsync(c->h_obs, c->d_obs, (size_t)c->replicas * sizeof(ReplicaObs), cudaMemcpyDeviceToHost, c->stream));
   IC_CUDA(cudaStreamSynchronize(c->stream));
   for (int r = 0; r < c->replicas; ++r) {
@@ -664,6 +678,7 @@ extern "C" int ic_observables(ic_ctx* c, ic_obs* h_out) {
 extern "C" int ic_debug_recompute(ic_ctx* c, int replica, int64_t* out6) {
   if (!c || !out6) return IC_ERR_NULL;
   if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  IC_ENTER(c);
   int rc = recompute_into_scratch(c, replica);
   if (rc != IC_OK) return rc;
   long long h[8];
@@ -691,6 +706,7 @@ extern "C" int ic_sweep_maps(ic_ctx* c, const double* h_T, int64_t nmaps, int64_
     if (!(h_T[r] > 0.0) || !std::isfinite(h_T[r])) return IC_ERR_PARAM;
   if (!d_scratch || scratch_bytes < ic_maps_scratch_bytes(c->L, K) || ((uintptr_t)d_scratch & 255) != 0) return IC_ERR_WORKSPACE;
   if (nmaps == 0) return IC_OK;
+  IC_ENTER(c);
   { int rc = ensure_thresholds(c, h_T); if (rc != IC_OK) return rc; }
   MapArgs a;
   a.lattice = c->lattice; a.thr = c->d_thr; a.obs = c->d_obs; a.lat_stride = c->lat_stride;
@@ -728,6 +744,7 @@ extern "C" int ic_largest_cluster(ic_ctx* c, int replica, int which, void* d_scr
   if (replica < 0 || replica >= c->replicas || !small_index_ok(c)) return IC_ERR_SIZE;
   if (which < 0 || which > 2) return IC_ERR_PARAM;
   if (!d_scratch || scratch_bytes < ic_cluster_scratch_bytes(c->L) || ((uintptr_t)d_scratch & 255) != 0) return IC_ERR_WORKSPACE;
+  IC_ENTER(c);
   int* parent = (int*)d_scratch; int* size = parent + c->N; long long* out2 = (long long*)(size + c->N);
   const LatView lat{c->lattice + (long long)replica * c->lat_stride, c->L, c->logL};
   const int nb = (int)std::min<long long>((c->N + 255) / 256, (long long)c->sm_count * 8);

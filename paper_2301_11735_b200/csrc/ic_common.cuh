@@ -142,6 +142,11 @@ constexpr int THR_STRIDE = 3520;         // table entries per replica (>= 3 * CL
 // y = packed (dn2, dV, dJ) = dJ + (dV << 11) + (dn2 << 22) for the per-thread observable accumulator.
 IC_HD int pack_delta(int dn2, int dV, int dJ) { return dJ + dV * 2048 + dn2 * 4194304; }
 IC_HD int class_index(int dn2, int dV, int dJ) { return (dn2 / 2 + 1) * CLS_SA + (dV + 16) * CLS_SB + (dJ + 16); }
+// Proposals that change nothing (abs(q) = 2, the current configuration, words 6 and 7 of a q = 0 pair) get a class entry of
+// their own with threshold 0: "never accepted" instead of "dE = 0, always accepted".  The lattice cannot tell the
+// difference; the kernels can: such lanes then skip the predicated second lookup and the write of the (empty) change.
+constexpr int NULL_CLASS = 3 * CLS_SA;   // first entry after the real classes; its bank holds no frequent class
+static_assert(NULL_CLASS < THR_STRIDE, "the null entry lies inside the table");
 IC_HD int class_index_public(int dn2, int dV, int dJ) { return ((dn2 / 2 + 1) * 33 + (dV + 16)) * 33 + (dJ + 16); }
 
 // Per-replica record in device memory: exact integers, then the fp64 sums of U5.
