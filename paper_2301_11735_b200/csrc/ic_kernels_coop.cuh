@@ -130,82 +130,80 @@ template <int BITS>
 __device__ __forceinline__ void coop_item(uint8_t* lat, int lw, int type, int p1, int p2, int phase, int wi, int hi, int half, int Y,
                                           uint32_t c2, uint32_t c3, uint32_t key0, uint32_t key1, uint32_t s_desc,
                                           int& tn2, int& tV, int& tJ, int& tM, int& tMs) {
-  const int W = 1 << lw, Wm = W - 1;
+  const int W = 1 << lw, Wm = W - 1, Lm = 4 * W - 1;
   const int Xj = 4 * wi, X0 = Xj & ~15, j = wi & 3;                  // plane column of the item's first pair; its 16-site vector; word in it
   uint32_t A4, B4, EA4, EB4, c0;
-  int a3 = 0, sgn, y;
-  auto R = [lw](int ky, int kx, int Yq) -> int { return ((Yq << 4) + (ky << 2) + kx) << lw; };   // plane row (lw <= 8: one tile per row quad)
+  int a3 = 0, sgn, ya;
+  // plane row kx of lattice row y (one tile per row quad: (y >> 2) * 16 + (y & 3) * 4 + kx = 4 y + kx plane rows of W sites)
+  auto R = [lw](int y, int kx) -> int { return ((y << 2) + kx) << lw; };
   if (type == 0) {
-    // ---- FAR: a = (ky, kxa) of row quad Y, b = its partner under (x ^ mx, y ^ my); eq. (4) ----------------------
+    // ---- FAR: a = (even x, y), b = its partner (x ^ mx, y ^ my); eq. (4) ------------------------------------------
     const int mx = p1, my = p2;
-    const int ky = phase + 2 * half, kxa = 2 * hi, kyb = ky ^ (my & 3), kxb = kxa ^ (mx & 3), Yb = Y ^ (my >> 2);
+    const int kxa = 2 * hi, kxb = kxa ^ (mx & 3);
+    ya = 4 * Y + phase + 2 * half;
+    const int yb = ya ^ my;
     // b in a's lane order: lane i <-> i ^ c, c = (mx >> 2) & 15: word j of the permuted vector is word j ^ (c >> 2)
     // of the partner chunk, its bytes permuted by c & 3
     const int jb = j ^ (((mx >> 2) & 15) >> 2), Xb0 = X0 ^ ((mx >> 2) & Wm & ~15), Xb = Xb0 + 4 * jb;
     const uint32_t selb = 0x3210u ^ (0x1111u * (uint32_t)((mx >> 2) & 3));
-    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
-    const int kybu = (kyb - 1) & 3, Ybu = (Yb - (kyb == 0)) & Wm, kybd = (kyb + 1) & 3, Ybd = (Yb + (kyb == 3)) & Wm;
-    const int ra = R(ky, kxa, Y), rb = R(kyb, kxb, Yb);
+    const int ra = R(ya, kxa), rb = R(yb, kxb);
     A4 = ldw<BITS>(lat, ra, Xj);
     const uint32_t b0 = ldw<BITS>(lat, rb, Xb);
-    EA4 = ldw_sh<BITS>(lat, R(ky, (kxa + 3) & 3, Y), Xj, W, kxa == 0 ? -1 : 0) + ldw<BITS>(lat, R(ky, kxa + 1, Y), Xj) +
-          ldw<BITS>(lat, R(kyu, kxa, Yu), Xj) + ldw<BITS>(lat, R(kyd, kxa, Yd), Xj);
-    const uint32_t eb0 = ldw<BITS>(lat, R(kyb, kxb - 1, Yb), Xb) + ldw_sh<BITS>(lat, R(kyb, (kxb + 1) & 3, Yb), Xb, W, kxb == 3 ? 1 : 0) +
-                         ldw<BITS>(lat, R(kybu, kxb, Ybu), Xb) + ldw<BITS>(lat, R(kybd, kxb, Ybd), Xb);
+    EA4 = ldw_sh<BITS>(lat, R(ya, (kxa + 3) & 3), Xj, W, kxa == 0 ? -1 : 0) + ldw<BITS>(lat, R(ya, kxa + 1), Xj) +
+          ldw<BITS>(lat, R((ya - 1) & Lm, kxa), Xj) + ldw<BITS>(lat, R((ya + 1) & Lm, kxa), Xj);
+    const uint32_t eb0 = ldw<BITS>(lat, R(yb, kxb - 1), Xb) + ldw_sh<BITS>(lat, R(yb, (kxb + 1) & 3), Xb, W, kxb == 3 ? 1 : 0) +
+                         ldw<BITS>(lat, R((yb - 1) & Lm, kxb), Xb) + ldw<BITS>(lat, R((yb + 1) & Lm, kxb), Xb);
     B4 = __byte_perm(b0, 0u, selb); EB4 = __byte_perm(eb0, 0u, selb);
-    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kxa);
-    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    c0 = (uint32_t)(4 * wi + kxa);
+    const u32x4 rr = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
     pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
     st_word<BITS>(lat, ra, X0, j, A4);
     st_word<BITS>(lat, rb, Xb0, jb, __byte_perm(B4, 0u, selb));
-    sgn = phase ? -1 : 1;
-    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-    tM += Ma + Mb; tMs += sgn * (Ma + Mb);
+    sgn = phase ? -2 : 2;                                            // both sites have the phase's colour
   } else if (p1 == 1) {
-    // ---- NEAR, vertical dominoes: a = (ky, kx), b = the site below; eq. (5) --------------------------------------
-    const int kx = half + 2 * hi, ky = (p2 + 2 * ((half + phase) & 1)) & 3;
-    const int kyb = (ky + 1) & 3, Yb = (Y + (ky == 3)) & Wm;
-    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (kyb + 1) & 3, Yd = (Yb + (kyb == 3)) & Wm;
-    const int ra = R(ky, kx, Y), rb = R(kyb, kx, Yb);
+    // ---- NEAR, vertical dominoes: a = (x, y), b = the site below; eq. (5) ------------------------------------------
+    const int kx = half + 2 * hi;
+    ya = 4 * Y + ((p2 + 2 * ((half + phase) & 1)) & 3);
+    const int yb = (ya + 1) & Lm;
+    const int ra = R(ya, kx), rb = R(yb, kx);
     const int shl = kx == 0 ? -1 : 0, shr = kx == 3 ? 1 : 0;
     A4 = ldw<BITS>(lat, ra, Xj); B4 = ldw<BITS>(lat, rb, Xj);
     // vertical domino: a's lower neighbour is b, b's upper neighbour is a
-    EA4 = ldw_sh<BITS>(lat, R(ky, (kx + 3) & 3, Y), Xj, W, shl) + ldw_sh<BITS>(lat, R(ky, (kx + 1) & 3, Y), Xj, W, shr) +
-          ldw<BITS>(lat, R(kyu, kx, Yu), Xj) + B4;
-    EB4 = ldw_sh<BITS>(lat, R(kyb, (kx + 3) & 3, Yb), Xj, W, shl) + ldw_sh<BITS>(lat, R(kyb, (kx + 1) & 3, Yb), Xj, W, shr) +
-          A4 + ldw<BITS>(lat, R(kyd, kx, Yd), Xj);
-    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kx);
-    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    EA4 = ldw_sh<BITS>(lat, R(ya, (kx + 3) & 3), Xj, W, shl) + ldw_sh<BITS>(lat, R(ya, (kx + 1) & 3), Xj, W, shr) +
+          ldw<BITS>(lat, R((ya - 1) & Lm, kx), Xj) + B4;
+    EB4 = ldw_sh<BITS>(lat, R(yb, (kx + 3) & 3), Xj, W, shl) + ldw_sh<BITS>(lat, R(yb, (kx + 1) & 3), Xj, W, shr) +
+          A4 + ldw<BITS>(lat, R((yb + 1) & Lm, kx), Xj);
+    c0 = (uint32_t)(4 * wi + kx);
+    const u32x4 rr = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
     pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
     st_word<BITS>(lat, ra, X0, j, A4);
     st_word<BITS>(lat, rb, X0, j, B4);
-    sgn = ((kx + ky) & 1) ? -1 : 1;
-    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-    tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+    sgn = ((kx + ya) & 1) ? -1 : 1;                                  // a and b have opposite colours
   } else {
-    // ---- NEAR, horizontal dominoes of row ky = half + 2 hi; lanes are indexed by the b-site; eq. (5) ------------
-    const int ky = half + 2 * hi;
+    // ---- NEAR, horizontal dominoes of row y; lanes are indexed by the b-site; eq. (5) ------------------------------
+    ya = 4 * Y + half + 2 * hi;
     const int ka = (p2 + 2 * ((half + phase) & 1)) & 3, kb = (ka + 1) & 3;
     const int sh_a = -(ka == 3), sh_l = sh_a - (ka == 0), sh_r = (kb == 3);
-    const int kyu = (ky - 1) & 3, Yu = (Y - (ky == 0)) & Wm, kyd = (ky + 1) & 3, Yd = (Y + (ky == 3)) & Wm;
-    const int ra = R(ky, ka, Y), rb = R(ky, kb, Y);
+    const int yu = (ya - 1) & Lm, yd = (ya + 1) & Lm;
+    const int ra = R(ya, ka), rb = R(ya, kb);
     A4 = ldw_sh<BITS>(lat, ra, Xj, W, sh_a); B4 = ldw<BITS>(lat, rb, Xj);
-    EA4 = ldw_sh<BITS>(lat, R(ky, (ka + 3) & 3, Y), Xj, W, sh_l) + B4 +
-          ldw_sh<BITS>(lat, R(kyu, ka, Yu), Xj, W, sh_a) + ldw_sh<BITS>(lat, R(kyd, ka, Yd), Xj, W, sh_a);
-    EB4 = A4 + ldw_sh<BITS>(lat, R(ky, (kb + 1) & 3, Y), Xj, W, sh_r) +
-          ldw<BITS>(lat, R(kyu, kb, Yu), Xj) + ldw<BITS>(lat, R(kyd, kb, Yd), Xj);
+    EA4 = ldw_sh<BITS>(lat, R(ya, (ka + 3) & 3), Xj, W, sh_l) + B4 +
+          ldw_sh<BITS>(lat, R(yu, ka), Xj, W, sh_a) + ldw_sh<BITS>(lat, R(yd, ka), Xj, W, sh_a);
+    EB4 = A4 + ldw_sh<BITS>(lat, R(ya, (kb + 1) & 3), Xj, W, sh_r) + ldw<BITS>(lat, R(yu, kb), Xj) + ldw<BITS>(lat, R(yd, kb), Xj);
     const uint32_t A4old = A4;
-    y = 4 * Y + ky; c0 = (uint32_t)(4 * wi + kb);
-    const u32x4 rr = philox_update(c0, (uint32_t)y, c2, c3, key0, key1);
+    c0 = (uint32_t)(4 * wi + kb);
+    const u32x4 rr = philox_update(c0, (uint32_t)ya, c2, c3, key0, key1);
     pairs4(A4, B4, EA4, EB4, rr.v[0], rr.v[1], rr.v[2], rr.v[3], s_desc, a3);
     st_word<BITS>(lat, rb, X0, j, B4);
     if (sh_a == 0) st_word<BITS>(lat, ra, X0, j, A4); else st_word_left1<BITS>(lat, ra, X0, W, j, A4, A4old);
-    sgn = ((ka + ky) & 1) ? -1 : 1;
-    const int Ma = (9 * __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)A4, 0x01010101, 0)) >> 3;
-    const int Mb = (9 * __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0) - __dp4a((int)B4, 0x01010101, 0)) >> 3;
-    tM += Ma + Mb; tMs += sgn * (Ma - Mb);
+    sgn = ((ka + ya) & 1) ? -1 : 1;
+  }
+  // M and Ms of the eight sites from their new bytes f | g<<3: sum sigma = sum f - sum g = (9 sum f - sum (f + 8 g)) / 8
+  {
+    const int Fa = __dp4a((int)(A4 & 0x07070707u), 0x01010101, 0), Fb = __dp4a((int)(B4 & 0x07070707u), 0x01010101, 0);
+    const int Ma = (9 * Fa - __dp4a((int)A4, 0x01010101, 0)) >> 3, Mb = (9 * Fb - __dp4a((int)B4, 0x01010101, 0)) >> 3;
+    tM += Ma + Mb;
+    tMs += (sgn & 1) ? sgn * (Ma - Mb) : (sgn >> 1) * (Ma + Mb);
   }
   // unpack the item's sums: a3 = dJ + (dV << 11) + (dn2 << 22)
   const int j11 = (a3 << 21) >> 21; a3 = (a3 - j11) >> 11;
