@@ -482,7 +482,8 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   // latency-bound: spread the items of a phase over as many SMs as there are, at least four warps per block
   const long long cap = blocks_cap(c, std::max<long long>(1, c->sm_count / c->replicas));
   const long long nblk = std::min(cap, (items + 127) / 128);
-  const int threads = (int)std::min<long long>(COOP_THREADS, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
+  // item threads per block + the service warp
+  const int threads = 32 + (int)std::min<long long>(COOP_THREADS - 32, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
   dim3 grid((unsigned)nblk, (unsigned)c->replicas);
   IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
   void* args[] = {(void*)&a};
@@ -504,7 +505,7 @@ static int launch_resvec(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   a.lat_stride = c->lat_stride; a.nsweeps = nsweeps; a.sweep0 = c->sweep; a.delta = c->delta; a.V = c->V; a.quarterJ = 0.25 * c->J;
   a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const long long items = c->N / 16;
-  const int threads = (int)std::min<long long>(COOP_THREADS, std::max<long long>(64, (items + 31) / 32 * 32));
+  const int threads = 32 + (int)std::min<long long>(COOP_THREADS - 32, std::max<long long>(32, (items + 31) / 32 * 32));   // + the service warp
   k_resvec_sweeps<LAYG><<<c->replicas, threads, RESV_SMEM_BYTES, c->stream>>>(a);
   c->launches++;
   IC_CUDA(cudaGetLastError());

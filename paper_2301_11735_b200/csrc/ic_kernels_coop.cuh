@@ -211,94 +211,115 @@ __device__ __forceinline__ void coop_item(uint8_t* lat, int lw, int type, int p1
   tJ += j11; tV += v11; tn2 += a3;
 }
 
+// ---- pieces shared by the two one-launch kernels -------------------------------------------------------------------------
+// class tables and per-lane move descriptors of both sweep types into shared memory (once per launch)
+__device__ __forceinline__ void fill_item_tables(unsigned char* smem, uint32_t smem0, const uint2* thr_r, const uint2* desc32, int tid, int nthr) {
+  uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
+  for (int k = tid; k < THR_STRIDE; k += nthr) { const uint2 v = __ldg(&thr_r[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+  uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
+  for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += nthr) {
+    const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
+    const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
+    uint2 d = __ldg(&desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
+    d.y += smem0 + COOP_OFF_THR;                // low 16 bits: shared-memory address of the class base
+    desc_s[k] = d;
+  }
+}
+// U4: parameters of a sweep, the same for all replicas (identical maps for all copies)
+__device__ __forceinline__ void sweep_schedule(int L, unsigned long long sweep, uint32_t key0, uint32_t key1, int* par) {
+  const u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, key0, key1);
+  if ((sweep & 1) == 0) { par[0] = 0; par[1] = (int)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); par[2] = (int)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1); }
+  else { par[0] = 1; par[1] = (int)(z.v[0] & 1u); par[2] = (int)(z.v[1] & 3u); }
+}
+// U5 for one sweep: the integers are current; one rounding per operation, the order of k_fold
+__device__ __forceinline__ void fold_sweep(ReplicaObs& o, double delta, double V, double quarterJ, long long* trace_row) {
+  const double E = __dadd_rn(__dadd_rn(__dmul_rn(delta, (double)o.n2), __dmul_rn(V, (double)o.bV)), __dmul_rn(quarterJ, (double)o.bJ));
+  const double M = (double)o.M, Ms = (double)o.Ms;
+  o.sumE = __dadd_rn(o.sumE, E); o.sumE2 = __dadd_rn(o.sumE2, __dmul_rn(E, E));
+  o.sumM = __dadd_rn(o.sumM, M); o.sumM2 = __dadd_rn(o.sumM2, __dmul_rn(M, M)); o.sumAbsM = __dadd_rn(o.sumAbsM, fabs(M));
+  o.sumMs = __dadd_rn(o.sumMs, Ms); o.sumMs2 = __dadd_rn(o.sumMs2, __dmul_rn(Ms, Ms)); o.sumAbsMs = __dadd_rn(o.sumAbsMs, fabs(Ms));
+  o.nmeas += 1;
+  if (trace_row) { trace_row[0] = o.n2; trace_row[1] = o.bV; trace_row[2] = o.bJ; trace_row[3] = o.M; trace_row[4] = o.Ms; trace_row[5] = o.Q; }
+}
+// the warp's sums of a sweep -> red[k][warp]
+__device__ __forceinline__ void warp_sums(int (*red)[COOP_THREADS / 32], int warp, int lane, int tn2, int tV, int tJ, int tM, int tMs) {
+  const unsigned full = 0xFFFFFFFFu;
+  tn2 = __reduce_add_sync(full, tn2); tV = __reduce_add_sync(full, tV); tJ = __reduce_add_sync(full, tJ);
+  tM = __reduce_add_sync(full, tM); tMs = __reduce_add_sync(full, tMs);
+  if (lane == 0) { red[0][warp] = tn2; red[1][warp] = tV; red[2][warp] = tJ; red[3][warp] = tM; red[4][warp] = tMs; }
+}
+
+// Both kernels run blockDim.x - 32 item threads and one SERVICE WARP (the last) that keeps everything serial off the
+// item threads' path: while they are in phase 0 of sweep s, its lane 0 derives the schedule of sweep s+1 and the warp adds up
+// the block's sums of sweep s-1 (written to red[(s-1)&1] before the barrier that ended that sweep); the fold of sweep s-1
+// (U5) follows.  All threads meet at the same barriers, two per sweep.
 template <int BITS>
 __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs A) {
   extern __shared__ __align__(128) unsigned char smem[];
-  __shared__ int s_par[4];
-  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31, nthr = (int)blockDim.x;
+  __shared__ int s_par[2][4];
+  __shared__ int red[2][5][COOP_THREADS / 32];
+  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nit = (int)blockDim.x - 32;
+  const bool service = tid >= nit;
   const uint32_t smem0 = smem_u32(smem);
-  {
-    const uint2* src = A.thr + (long long)r * THR_STRIDE;
-    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
-    for (int k = tid; k < THR_STRIDE; k += nthr) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
-    uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
-    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += nthr) {
-      const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
-      const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
-      uint2 d = __ldg(&A.desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
-      d.y += smem0 + COOP_OFF_THR;                // low 16 bits: shared-memory address of the class base
-      desc_s[k] = d;
-    }
-  }
+  fill_item_tables(smem, smem0, A.thr + (long long)r * THR_STRIDE, A.desc32, tid, (int)blockDim.x);
   const int L = A.L, lw = A.logL - 2;
   const int n_items = 1 << (2 * lw);                               // (row quad, half, hi, word of the plane row): N/16 items of 4 pairs
   uint8_t* lat = reinterpret_cast<uint8_t*>(A.lattice) + (long long)r * A.lat_stride;
   CoopScratch* sc = &A.scratch[r];
   const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
-  const bool folder = blockIdx.x == 0 && tid == 0;
+  const bool folder = blockIdx.x == 0 && tid == nit;              // lane 0 of the service warp of the replica's first block
   ReplicaObs o;
   if (folder) o = A.obs[r];
+  if (tid == nit) sweep_schedule(L, A.sweep0, A.key0, A.key1, s_par[0]);
   unsigned int bar_target = 0;
   __syncthreads();
 
+  // sums of sweep q: block -> the replica's accumulator acc[q & 1] (service warp); accumulator -> integers -> fold (folder)
+  auto push_sums = [&](long long q) {
+    const unsigned full = 0xFFFFFFFFu;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const int v = __reduce_add_sync(full, lane < (nit >> 5) ? red[q & 1][k][lane] : 0);
+      if (lane == 0 && v) atomicAdd((unsigned long long*)&sc->acc[q & 1][k], (unsigned long long)(long long)v);
+    }
+  };
+  auto fold = [&](long long q) {
+    volatile long long* va = sc->acc[q & 1];
+    o.n2 += va[0]; o.bV += va[1]; o.bJ += va[2]; o.M = va[3]; o.Ms = va[4];      // the two phases covered every site once
+    va[0] = 0; va[1] = 0; va[2] = 0; va[3] = 0; va[4] = 0;                       // next used for sweep q + 2, five barriers on
+    fold_sweep(o, A.delta, A.V, A.quarterJ, A.trace ? A.trace + 6LL * ((long long)A.replicas * q + r) : nullptr);
+  };
+
   for (long long s = 0; s < A.nsweeps; ++s) {
     const unsigned long long sweep = A.sweep0 + (unsigned long long)s;
-    if (tid == 0) {
-      // U4: parameters of the sweep, the same for all replicas (identical maps for all copies)
-      const u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, A.key0, A.key1);
-      if ((sweep & 1) == 0) { s_par[0] = 0; s_par[1] = (int)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); s_par[2] = (int)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1); }
-      else { s_par[0] = 1; s_par[1] = (int)(z.v[0] & 1u); s_par[2] = (int)(z.v[1] & 3u); }
-    }
-    __syncthreads();
-    const int type = s_par[0], p1 = s_par[1], p2 = s_par[2];
+    const int type = s_par[s & 1][0], p1 = s_par[s & 1][1], p2 = s_par[s & 1][2];
     const uint32_t s_desc = smem0 + COOP_OFF_DESC + (type ? ST_DESC_SMEM : 0) + (uint32_t)(lane & 15) * 8u;
-    long long* acc = sc->acc[s & 1];
-
     int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;       // this thread's sums over both phases of the sweep
     for (int phase = 0; phase < 2; ++phase) {
-      const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
-      for (int it = blockIdx.x * nthr + tid; it < n_items; it += gridDim.x * nthr) {
-        int wi, hi, half, Y;
-        item_coords(it, lw, wi, hi, half, Y);
-        coop_item<BITS>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
-      }
-      // block sums -> the sweep's accumulator
-      if (phase == 1) {
-        __shared__ int red[5][COOP_THREADS / 32];
-        const unsigned full = 0xFFFFFFFFu;
-        tn2 = __reduce_add_sync(full, tn2); tV = __reduce_add_sync(full, tV); tJ = __reduce_add_sync(full, tJ);
-        tM = __reduce_add_sync(full, tM); tMs = __reduce_add_sync(full, tMs);
-        const int warp = tid >> 5;
-        if (lane == 0) { red[0][warp] = tn2; red[1][warp] = tV; red[2][warp] = tJ; red[3][warp] = tM; red[4][warp] = tMs; }
-        __syncthreads();
-        if (warp == 0) {
-#pragma unroll
-          for (int k = 0; k < 5; ++k) {
-            const int v = __reduce_add_sync(full, lane < (nthr >> 5) ? red[k][lane] : 0);
-            if (lane == 0 && v) atomicAdd((unsigned long long*)&acc[k], (unsigned long long)(long long)v);
-          }
+      if (!service) {
+        const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
+        for (int it = blockIdx.x * nit + tid; it < n_items; it += gridDim.x * nit) {
+          int wi, hi, half, Y;
+          item_coords(it, lw, wi, hi, half, Y);
+          coop_item<BITS>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
         }
+        if (phase == 1) warp_sums(red[s & 1], warp, lane, tn2, tV, tJ, tM, tMs);
+      } else if (phase == 0) {
+        if (lane == 0) sweep_schedule(L, sweep + 1, A.key0, A.key1, s_par[(s + 1) & 1]);
+        if (s > 0) push_sums(s - 1);      // complete in every block before its arrival at the barrier below
+      } else if (folder && s > 0) {
+        fold(s - 1);                      // all blocks have passed the barrier after phase 0: the accumulator is complete
       }
       bar_target += gridDim.x;
-      coop_barrier(&sc->arrived, bar_target);       // phase 1 reads neighbours written in phase 0; the fold reads all sums
+      coop_barrier(&sc->arrived, bar_target);       // phase 1 reads neighbours written in phase 0, and the next sweep those of phase 1
     }
-    if (folder) {
-      volatile long long* va = acc;
-      o.n2 += va[0]; o.bV += va[1]; o.bJ += va[2]; o.M = va[3]; o.Ms = va[4];    // the two phases covered every site once
-      va[0] = 0; va[1] = 0; va[2] = 0; va[3] = 0; va[4] = 0;                     // reused two sweeps (four barriers) from now
-      // U5, one rounding per operation, the order of k_fold
-      const double E = __dadd_rn(__dadd_rn(__dmul_rn(A.delta, (double)o.n2), __dmul_rn(A.V, (double)o.bV)),
-                                 __dmul_rn(A.quarterJ, (double)o.bJ));
-      const double M = (double)o.M, Ms = (double)o.Ms;
-      o.sumE = __dadd_rn(o.sumE, E); o.sumE2 = __dadd_rn(o.sumE2, __dmul_rn(E, E));
-      o.sumM = __dadd_rn(o.sumM, M); o.sumM2 = __dadd_rn(o.sumM2, __dmul_rn(M, M)); o.sumAbsM = __dadd_rn(o.sumAbsM, fabs(M));
-      o.sumMs = __dadd_rn(o.sumMs, Ms); o.sumMs2 = __dadd_rn(o.sumMs2, __dmul_rn(Ms, Ms)); o.sumAbsMs = __dadd_rn(o.sumAbsMs, fabs(Ms));
-      o.nmeas += 1;
-      if (A.trace) {
-        long long* tr = A.trace + 6LL * ((long long)A.replicas * s + r);
-        tr[0] = o.n2; tr[1] = o.bV; tr[2] = o.bJ; tr[3] = o.M; tr[4] = o.Ms; tr[5] = o.Q;
-      }
-    }
+  }
+  // the last sweep's sums
+  if (A.nsweeps > 0) {
+    if (service) push_sums(A.nsweeps - 1);
+    bar_target += gridDim.x;
+    coop_barrier(&sc->arrived, bar_target);
+    if (folder) fold(A.nsweeps - 1);
   }
   if (folder) A.obs[r] = o;
 }
@@ -307,7 +328,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
 // Small lattices (16 <= L <= 64, configs C1 and C2): the same items with the replica's lattice resident in shared memory.
 // One block per replica runs all the sweeps of an ic_sweep call; the lattice is converted from its layout in global memory
 // (LAYG: ROW8, ROW2 or P16) to P16 bytes on the way in and back on the way out, the phases are separated by
-// __syncthreads, thread 0 folds the sweep (U5).
+// __syncthreads, lane 0 of the service warp folds sweep s-1 (U5) while the item threads are in phase 0 of sweep s.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int RESV_MIN_L = 16, RESV_MAX_L = 64;
 constexpr int RESV_OFF_LAT = COOP_SMEM_BYTES;
@@ -316,82 +337,54 @@ constexpr int RESV_SMEM_BYTES = RESV_OFF_LAT + RESV_MAX_L * RESV_MAX_L;
 template <int LAYG>
 __global__ void __launch_bounds__(COOP_THREADS, 1) k_resvec_sweeps(const CoopArgs A) {
   extern __shared__ __align__(128) unsigned char smem[];
-  __shared__ int s_par[4];
-  __shared__ int red[5][COOP_THREADS / 32];
-  const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, nthr = (int)blockDim.x;
+  __shared__ int s_par[2][4];
+  __shared__ int red[2][5][COOP_THREADS / 32];
+  const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = (int)blockDim.x, nit = nthr - 32;
+  const bool service = tid >= nit;
   const uint32_t smem0 = smem_u32(smem);
   const int L = A.L, logL = A.logL, lw = logL - 2, N = L * L;
   const LatView gv{(char*)A.lattice + (long long)r * A.lat_stride, L, logL};
   uint8_t* lat = smem + RESV_OFF_LAT;
-  {
-    const uint2* src = A.thr + (long long)r * THR_STRIDE;
-    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + COOP_OFF_THR);
-    for (int k = tid; k < THR_STRIDE; k += nthr) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
-    uint2* desc_s = reinterpret_cast<uint2*>(smem + COOP_OFF_DESC);
-    for (int k = tid; k < 2 * ST_DESC_SMEM / 8; k += nthr) {
-      const int adj = k >= ST_DESC_SMEM / 8, kk = adj ? k - ST_DESC_SMEM / 8 : k;
-      const int row = kk >> 4, rr = row / 28, key = row - 28 * rr;
-      uint2 d = __ldg(&A.desc32[adj * ST_DESC_ENTRIES + key * 8 + rr]);
-      d.y += smem0 + COOP_OFF_THR;
-      desc_s[k] = d;
-    }
-    for (int i = tid; i < N; i += nthr) {
-      const int x = i & (L - 1), y = i >> logL;
-      lat[p16_site(lw, x, y)] = (uint8_t)e_of_code(Sites<LAYG>::load(gv, x, y));
-    }
+  fill_item_tables(smem, smem0, A.thr + (long long)r * THR_STRIDE, A.desc32, tid, nthr);
+  for (int i = tid; i < N; i += nthr) {
+    const int x = i & (L - 1), y = i >> logL;
+    lat[p16_site(lw, x, y)] = (uint8_t)e_of_code(Sites<LAYG>::load(gv, x, y));
   }
   const int n_items = 1 << (2 * lw);
   const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
   ReplicaObs o;
-  if (tid == 0) o = A.obs[r];
+  if (tid == nit) { o = A.obs[r]; sweep_schedule(L, A.sweep0, A.key0, A.key1, s_par[0]); }
   __syncthreads();
+
+  auto fold = [&](long long q) {          // lane 0 of the service warp: block sums of sweep q -> integers -> U5
+    long long M = 0, Ms = 0;
+    for (int wv = 0; wv < (nit >> 5); ++wv) { o.n2 += red[q & 1][0][wv]; o.bV += red[q & 1][1][wv]; o.bJ += red[q & 1][2][wv]; M += red[q & 1][3][wv]; Ms += red[q & 1][4][wv]; }
+    o.M = M; o.Ms = Ms;                   // the two phases covered every site once
+    fold_sweep(o, A.delta, A.V, A.quarterJ, A.trace ? A.trace + 6LL * ((long long)A.replicas * q + r) : nullptr);
+  };
 
   for (long long s = 0; s < A.nsweeps; ++s) {
     const unsigned long long sweep = A.sweep0 + (unsigned long long)s;
-    if (tid == 0) {
-      // U4: parameters of the sweep, the same for all replicas (identical maps for all copies)
-      const u32x4 z = philox4x32_10(0u, 0u, (uint32_t)sweep, TAG_SCHED << 28, A.key0, A.key1);
-      if ((sweep & 1) == 0) { s_par[0] = 0; s_par[1] = (int)(2 * (z.v[0] & (uint32_t)(L / 2 - 1)) + 1); s_par[2] = (int)(2 * (z.v[1] & (uint32_t)(L / 2 - 1)) + 1); }
-      else { s_par[0] = 1; s_par[1] = (int)(z.v[0] & 1u); s_par[2] = (int)(z.v[1] & 3u); }
-    }
-    __syncthreads();
-    const int type = s_par[0], p1 = s_par[1], p2 = s_par[2];
+    const int type = s_par[s & 1][0], p1 = s_par[s & 1][1], p2 = s_par[s & 1][2];
     const uint32_t s_desc = smem0 + COOP_OFF_DESC + (type ? ST_DESC_SMEM : 0) + (uint32_t)(lane & 15) * 8u;
     int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
     for (int phase = 0; phase < 2; ++phase) {
-      const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
-      for (int it = tid; it < n_items; it += nthr) {
-        int wi, hi, half, Y;
-        item_coords(it, lw, wi, hi, half, Y);
-        coop_item<8>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
+      if (!service) {
+        const uint32_t c2 = (uint32_t)(2 * sweep + (unsigned long long)phase);
+        for (int it = tid; it < n_items; it += nit) {
+          int wi, hi, half, Y;
+          item_coords(it, lw, wi, hi, half, Y);
+          coop_item<8>(lat, lw, type, p1, p2, phase, wi, hi, half, Y, c2, c3, A.key0, A.key1, s_desc, tn2, tV, tJ, tM, tMs);
+        }
+        if (phase == 1) warp_sums(red[s & 1], warp, lane, tn2, tV, tJ, tM, tMs);
+      } else if (phase == 0 && tid == nit) {
+        sweep_schedule(L, sweep + 1, A.key0, A.key1, s_par[(s + 1) & 1]);
+        if (s > 0) fold(s - 1);           // red[(s-1)&1] was complete at the barrier that ended sweep s-1; rewritten in sweep s+1
       }
-      __syncthreads();       // phase 1 reads neighbours written in phase 0
+      __syncthreads();       // phase 1 reads neighbours written in phase 0, and the next sweep those of phase 1
     }
-    const unsigned full = 0xFFFFFFFFu;
-    tn2 = __reduce_add_sync(full, tn2); tV = __reduce_add_sync(full, tV); tJ = __reduce_add_sync(full, tJ);
-    tM = __reduce_add_sync(full, tM); tMs = __reduce_add_sync(full, tMs);
-    if (lane == 0) { const int warp = tid >> 5; red[0][warp] = tn2; red[1][warp] = tV; red[2][warp] = tJ; red[3][warp] = tM; red[4][warp] = tMs; }
-    __syncthreads();
-    if (tid == 0) {
-      long long M = 0, Ms = 0;
-      for (int wv = 0; wv < (nthr >> 5); ++wv) { o.n2 += red[0][wv]; o.bV += red[1][wv]; o.bJ += red[2][wv]; M += red[3][wv]; Ms += red[4][wv]; }
-      o.M = M; o.Ms = Ms;                                  // the two phases covered every site once
-      // U5, one rounding per operation, the order of k_fold
-      const double E = __dadd_rn(__dadd_rn(__dmul_rn(A.delta, (double)o.n2), __dmul_rn(A.V, (double)o.bV)),
-                                 __dmul_rn(A.quarterJ, (double)o.bJ));
-      const double Md = (double)o.M, Msd = (double)o.Ms;
-      o.sumE = __dadd_rn(o.sumE, E); o.sumE2 = __dadd_rn(o.sumE2, __dmul_rn(E, E));
-      o.sumM = __dadd_rn(o.sumM, Md); o.sumM2 = __dadd_rn(o.sumM2, __dmul_rn(Md, Md)); o.sumAbsM = __dadd_rn(o.sumAbsM, fabs(Md));
-      o.sumMs = __dadd_rn(o.sumMs, Msd); o.sumMs2 = __dadd_rn(o.sumMs2, __dmul_rn(Msd, Msd)); o.sumAbsMs = __dadd_rn(o.sumAbsMs, fabs(Msd));
-      o.nmeas += 1;
-      if (A.trace) {
-        long long* tr = A.trace + 6LL * ((long long)A.replicas * s + r);
-        tr[0] = o.n2; tr[1] = o.bV; tr[2] = o.bJ; tr[3] = o.M; tr[4] = o.Ms; tr[5] = o.Q;
-      }
-    }
-    // red is rewritten only after the three barriers of the next sweep
   }
-  __syncthreads();
+  if (tid == nit && A.nsweeps > 0) fold(A.nsweeps - 1);
   // the lattice goes back in its layout
   if (LAYG == LAY_ROW2) {
     uint32_t* words = reinterpret_cast<uint32_t*>(gv.base);
@@ -407,7 +400,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_resvec_sweeps(const CoopArg
   } else {
     for (int i = tid; i < N; i += nthr) ((uint8_t*)gv.base)[i] = lat[i];
   }
-  if (tid == 0) A.obs[r] = o;
+  if (tid == nit) A.obs[r] = o;
 }
 
 }  // namespace ic
