@@ -336,6 +336,27 @@ def test_config_c5_full_size_sampled(pkg, bits):
     sim.close()
 
 
+def test_variant_and_block_bound_argument_checks(pkg):
+    """ic_set_variant refuses a kernel family that cannot run the context's (L, bits); ic_set_max_blocks a negative bound."""
+    small = pkg.Sim(64, 0.1, 0.5, 1.0, 1.0, seed=1)
+    for bad in (2 + 1, 5, 7, -1):                  # staged and one-launch kernels need L >= 2048 / 128; 7 does not exist
+        with pytest.raises(pkg.IcError) as e:
+            small.set_variant(bad)
+        assert e.value.code == pkg.IC_ERR_PARAM
+    for ok in (0, 1, 2, 4, 6):
+        small.set_variant(ok)
+    with pytest.raises(pkg.IcError):
+        small.set_max_blocks(-1)
+    small.set_max_blocks(3); small.set_max_blocks(0)
+    small.close()
+    mid = pkg.Sim(256, 0.1, 0.5, 1.0, 1.0, seed=1, bits_per_site=2)
+    for bad in (2, 3, 4, 6):                       # tiled kernels are 8 bits/site only; resident kernels need L <= 64
+        with pytest.raises(pkg.IcError):
+            mid.set_variant(bad)
+    mid.set_variant(5); mid.set_variant(1); mid.set_variant(0)
+    mid.close()
+
+
 def test_staged_kernels_one_block_per_replica(pkg):
     """More replicas than SMs: the staged kernels run with gridDim.x = 1 (one persistent block per replica walks the whole
     lattice).  L=2048, 160 replicas; three replicas against the oracle, every replica against eq. (2) and the recount."""
