@@ -156,7 +156,7 @@ int ic_snapshot_ppm(ic_ctx* ctx, int replica, const char* path);
  * runs all sweeps of an ic_sweep call in one launch, one thread per pair; the default for L < 16).
  * 6 = resident kernel with four-pair items (16 <= L <= 64, any bits_per_site: the same, with the item code of the staged
  * kernels on a byte lattice in shared memory; the default there).
- * 5 = one-launch kernel (8 or 2 bits/site, 128 <= L <= 1024, replicas <= number of SMs: one cooperative launch runs
+ * 5 = one-launch kernel (8 or 2 bits/site, 128 <= L <= 1024: one cooperative launch runs
  * all sweeps of an ic_sweep call on the whole GPU, the phases separated by a barrier over the replica's blocks; the
  * default there).
  * IC_ERR_PARAM if the variant cannot run this context's (L, bits_per_site).  All variants produce identical

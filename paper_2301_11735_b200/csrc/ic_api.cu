@@ -465,7 +465,7 @@ static int launch_staged_one(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
 }
 // one cooperative launch for all the sweeps of a call: single mid-size lattices (ic_kernels_coop.cuh)
 static bool coop_ok(const ic_ctx* c) {
-  return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= COOP_MIN_L && c->L <= COOP_MAX_L && c->replicas <= c->sm_count && c->coop_supported;
+  return (c->layout == LAY_P16 || c->layout == LAY_P2) && c->L >= COOP_MIN_L && c->L <= COOP_MAX_L && c->coop_supported;
 }
 template <int BITS>
 static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
@@ -480,11 +480,12 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   a.L = c->L; a.logL = c->logL; a.replicas = c->replicas; a.key0 = (uint32_t)c->seed; a.key1 = (uint32_t)(c->seed >> 32);
   const long long items = c->N / 16;                                   // four pairs per item, N/4 pairs per phase
   // latency-bound: spread the items of a phase over as many SMs as there are, at least four warps per block
-  const long long cap = blocks_cap(c, std::max<long long>(1, c->sm_count / c->replicas));
+  const int rows = std::min(c->replicas, c->sm_count);              // rows of blocks; a row takes every rows-th replica
+  const long long cap = blocks_cap(c, std::max<long long>(1, c->sm_count / rows));
   const long long nblk = std::min(cap, (items + 127) / 128);
   // item threads per block + the service warp
   const int threads = 32 + (int)std::min<long long>(COOP_THREADS - 32, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
-  dim3 grid((unsigned)nblk, (unsigned)c->replicas);
+  dim3 grid((unsigned)nblk, (unsigned)rows);
   IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
   void* args[] = {(void*)&a};
   IC_CUDA(cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream));

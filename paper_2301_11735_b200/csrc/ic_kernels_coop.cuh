@@ -258,12 +258,16 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ int s_par[2][4];
   __shared__ int red[2][5][COOP_THREADS / 32];
-  const int r = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nit = (int)blockDim.x - 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nit = (int)blockDim.x - 32;
   const bool service = tid >= nit;
   const uint32_t smem0 = smem_u32(smem);
-  fill_item_tables(smem, smem0, A.thr + (long long)r * THR_STRIDE, A.desc32, tid, (int)blockDim.x);
   const int L = A.L, lw = A.logL - 2;
   const int n_items = 1 << (2 * lw);                               // (row quad, half, hi, word of the plane row): N/16 items of 4 pairs
+  // a row of blocks (blockIdx.y) takes the replicas blockIdx.y, blockIdx.y + gridDim.y, ... one after the other, each for
+  // all the sweeps of the call (replicas are independent; more replicas than SMs is the only case with more than one)
+  for (int r = blockIdx.y; r < A.replicas; r += gridDim.y) {
+  __syncthreads();                                                 // the previous replica's tables are no longer read
+  fill_item_tables(smem, smem0, A.thr + (long long)r * THR_STRIDE, A.desc32, tid, (int)blockDim.x);
   uint8_t* lat = reinterpret_cast<uint8_t*>(A.lattice) + (long long)r * A.lat_stride;
   CoopScratch* sc = &A.scratch[r];
   const uint32_t c3 = (uint32_t)r | (TAG_UPDATE << 28);
@@ -322,6 +326,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
     if (folder) fold(A.nsweeps - 1);
   }
   if (folder) A.obs[r] = o;
+  }   // replicas of this row of blocks
 }
 
 // ---------------------------------------------------------------------------------------------------------------

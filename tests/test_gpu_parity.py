@@ -336,6 +336,30 @@ def test_config_c5_full_size_sampled(pkg, bits):
     sim.close()
 
 
+def test_one_launch_kernel_with_more_replicas_than_sms(pkg):
+    """More lattice copies than SMs at L = 128 (2 bits/site): every row of blocks of the one-launch kernel runs several
+    replicas one after the other.  Three replicas against the oracle, all against eq. (2) and the recount."""
+    import torch
+    L, reps, seed, nsw = 128, torch.cuda.get_device_properties(0).multi_processor_count + 9, 61, 12
+    Ts = [0.4 + 0.01 * r for r in range(reps)]
+    sim = pkg.Sim(L, 0.1, 0.5, 1.0, 1.0, seed=seed, replicas=reps, bits_per_site=2); sim.set_variant(5)
+    picks = [0, reps - 10, reps - 1]
+    codes = {r: sim.state(r).copy() for r in picks}
+    sim.sweep(Ts, nsw)
+    obs = sim.observables()
+    for r in picks:
+        lat = oracle.Lattice(codes[r], 0.5, 1.0, 1.0, seed, replica=r)
+        lat.sweep_s1(Ts[r], nsw)
+        assert np.array_equal(sim.state(r), lat.code), r
+        ref = lat.observables(Ts[r])
+        for k in ("n2", "bV", "bJ", "M", "Ms", "Q", "sumE", "sumE2", "nmeas"):
+            assert obs[r][k] == ref[k], (r, k)
+    for r in range(0, reps, 5):
+        assert obs[r]["Q"] == sim.Q and obs[r]["nmeas"] == nsw
+        assert list(sim.debug_recompute(r)) == [obs[r][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q")]
+    sim.close()
+
+
 def test_variant_and_block_bound_argument_checks(pkg):
     """ic_set_variant refuses a kernel family that cannot run the context's (L, bits); ic_set_max_blocks a negative bound."""
     small = pkg.Sim(64, 0.1, 0.5, 1.0, 1.0, seed=1)
