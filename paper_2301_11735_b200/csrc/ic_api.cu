@@ -488,7 +488,13 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   dim3 grid((unsigned)nblk, (unsigned)rows);
   IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
   void* args[] = {(void*)&a};
-  IC_CUDA(cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream));
+  const cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream);
+  if (e == cudaErrorCooperativeLaunchTooLarge) {   // fewer SMs available than the device reports (MPS, green contexts): per-phase kernels from now on
+    (void)cudaGetLastError();
+    c->coop_supported = false;
+    return 1;
+  }
+  IC_CUDA(e);
   c->launches++;
   return IC_OK;
 }
@@ -597,9 +603,9 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
   // single mid-size lattices: all the sweeps in one cooperative launch over the whole GPU
   if (coop_ok(c) && (c->variant == 0 || c->variant == 5)) {
     int rc = c->layout == LAY_P2 ? launch_coop<2>(c, nsweeps, d_trace) : launch_coop<8>(c, nsweeps, d_trace);
-    if (rc != IC_OK) return rc;
-    c->sweep += (uint64_t)nsweeps;
-    return IC_OK;
+    if (rc < 0) return rc;
+    if (rc == IC_OK) { c->sweep += (uint64_t)nsweeps; return IC_OK; }
+    if (c->variant == 5) c->variant = 0;           // rc > 0: the cooperative launch does not fit; fall through to the phase kernels
   }
 
   PhaseArgs a;
