@@ -4,14 +4,14 @@
 //
 // One launch = one phase of a sweep (schedule S1, U4), one persistent block per SM, launched as a programmatic
 // dependent of the previous kernel of the stream (table fill and barrier set-up overlap that kernel's tail):
-//   * 3 producer warps (the last three of the block), one per consumer group, stage "regions" of the lattice in shared
+//   * 2 producer warps (the last two of the block), one per consumer group, stage "regions" of the lattice in shared
 //     memory with 1-D bulk copies (cp.async.bulk, the TMA engine; completion on an mbarrier).  A region is one tile of
 //     the layout (row quad Y, 512 plane columns: 16 plane rows) plus the plane rows of the lattice row above and of the one
 //     (NEAR-V: two) below.  Tiles are stored in the order [segment][Y], so the whole region is ONE contiguous piece of
 //     12 KB (NEAR-V: 14 KB) and one bulk copy (two at the periodic wrap Y = 0 / Y = W-1).  The few bytes read across the
 //     left/right tile edge (the x-1 neighbour of plane 0 is plane 3 one byte to the left) are fetched by the producer's
 //     lanes with plain loads, issued a task ahead, into a small side array.
-//   * 24 consumer warps in 3 groups; group g processes tasks g, g+3, ... of the block and owns two stage slots
+//   * 16 consumer warps in 2 groups; group g processes tasks g, g+2, ... of the block and owns two stage slots
 //     (double buffering; a slot goes back to the producers as soon as the items are in registers).  A task is two
 //     regions = 4096 coupled pairs, a thread's item one 16-byte vector = 16 pairs.  In a FAR phase the two regions are
 //     partners under (x^mx, y^my): every byte of both is loaded once and all pairs between them are updated.
@@ -27,11 +27,14 @@
 
 namespace ic {
 
-constexpr int ST_GROUPS = 3;                  // consumer groups per block
+// Two groups of eight consumer warps: 18 warps per SM leave each thread the ~90 registers the item code wants (three groups at 72
+// registers: -1.5 % at C5, -2.7 % at C4; measured, profiles/r02d)
+constexpr int ST_GROUPS = 2;                  // consumer groups per block
+constexpr int ST_DEPTH = 2;                   // ring slots per consumer group
 constexpr int ST_NPROD = ST_GROUPS;           // producer warps per block: one per consumer group
 constexpr int ST_LOGSEG = P16_LOGSEG_MAX, ST_SEG = 1 << ST_LOGSEG;   // plane columns per region = per tile of the layout
 constexpr int ST_TPG = ST_SEG / 2;            // consumer threads per group: one 16-pair item each per task
-constexpr int ST_CONS = ST_GROUPS * ST_TPG;   // consumer threads (warps 0..23); the producers are warps 24..26
+constexpr int ST_CONS = ST_GROUPS * ST_TPG;   // consumer threads (warps 0..15); the producers are warps 16, 17
 constexpr int ST_THREADS = ST_CONS + 32 * ST_NPROD;
 constexpr int ST_DESC_ENTRIES = 256;          // move descriptors [key*8 + r] (224 used) in global memory: (coefficients, info)
 constexpr int ST_DESC_SMEM = 28 * 8 * 128;    // in shared memory: [r][key][lane & 15] x 8 bytes, a private copy per lane
@@ -55,7 +58,7 @@ struct StagedCfg {
   static constexpr int OFF_HALO = 2 * REGION_BYTES;                 // [2 regions][left, right][32 rows] edge entries
   static constexpr int OFF_SMETA = OFF_HALO + 128 * HE;             // SubMeta[4]
   static constexpr int STAGE_BYTES = OFF_SMETA + 128;
-  static constexpr int NSTAGE = 2 * ST_GROUPS;                      // slots 2g, 2g+1 belong to consumer group g
+  static constexpr int NSTAGE = ST_DEPTH * ST_GROUPS;               // slots ST_DEPTH g .. ST_DEPTH g + ST_DEPTH - 1 belong to consumer group g
   // dynamic shared memory map (byte offsets)
   static constexpr int OFF_THR = 0;                                 // uint32 threshold[THR_STRIDE], then uint32 packed deltas[THR_STRIDE]
   static constexpr int OFF_DESC = OFF_THR + THR_STRIDE * 8;         // uint2 descriptors [8][28][16]
@@ -237,7 +240,7 @@ __device__ __forceinline__ void st16_left1_tile(uint8_t* row, uint8_t* left, int
 
 // ---------------------------------------------------------------------------------------------------------------
 // The phase kernel.  TYPE: PH_FAR / PH_NEAR_H / PH_NEAR_V; CW: word part of the FAR lane permutation.
-// grid = (blocks, replicas), block = 3 groups of 256 consumer threads + 3 producer warps.
+// grid = (blocks, replicas), block = 2 groups of 256 consumer threads + 2 producer warps.
 // ---------------------------------------------------------------------------------------------------------------
 template <int TYPE, int CW, int BITS>
 __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_constant__ PhaseArgs A) {
@@ -292,7 +295,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
   // byte offset of the tile (Y, seg) in the lattice: tiles in the order [seg][Y], 16 plane rows of SEG bytes each
   auto tile_off = [&](int Y, int seg) -> long long { return ((((long long)seg << lw) + Y) << 4) * RB; };
   // tasks of this block: t = blockIdx.x + n * gridDim.x, n = 0, 1, ...; task n belongs to consumer group g = n % ST_GROUPS
-  // and is its k-th task, k = n / ST_GROUPS; it lives in slot 2 g + (k & 1) on lap (k >> 1) & 1.  A slot is thus always
+  // and is its k-th task, k = n / ST_GROUPS; it lives in slot ST_DEPTH g + k % ST_DEPTH on lap (k / ST_DEPTH) & 1.  A slot is thus always
   // drained by the same group and filled in task order, so nobody can wait on a barrier more than one phase away from
   // its own -- the only case a parity wait gets wrong.
   int tn2 = 0, tV = 0, tJ = 0, tM = 0, tMs = 0;
@@ -326,7 +329,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     const int tstep = ST_GROUPS * (int)gridDim.x;
     halo_load((int)blockIdx.x + g * (int)gridDim.x, hl, hr);
     for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += tstep, ++k) {
-      const int s = 2 * g + (k & 1), lap = (k >> 1) & 1;
+      const int kd = k % ST_DEPTH, s = ST_DEPTH * g + kd, lap = (k / ST_DEPTH) & 1;
       const uint32_t full = bar0 + 8 * s;
       int Yq[2], sg[2];
 #pragma unroll
@@ -450,14 +453,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       goffa = 8 * hi * RB; goffb = 8 * hi * RB + X0 * BITS / 8;        // plane rows (ky, ka), (ky, kb)
     }
     constexpr int ROW4 = 4 * RB;                                       // four staged rows = one lattice row up / down
-    const uint32_t stg_g = smem0 + C::OFF_STAGE + 2 * g * C::STAGE_BYTES;
-    const SubMeta* meta_g = reinterpret_cast<const SubMeta*>(smem + C::OFF_STAGE + 2 * g * C::STAGE_BYTES + C::OFF_SMETA) + sub;
+    const uint32_t stg_g = smem0 + C::OFF_STAGE + ST_DEPTH * g * C::STAGE_BYTES;
+    const SubMeta* meta_g = reinterpret_cast<const SubMeta*>(smem + C::OFF_STAGE + ST_DEPTH * g * C::STAGE_BYTES + C::OFF_SMETA) + sub;
 
     for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += ST_GROUPS * gridDim.x, ++k) {
-      const int s = 2 * g + (k & 1), lap = (k >> 1) & 1;
-      const uint32_t st = stg_g + (k & 1) * C::STAGE_BYTES;
+      const int kd = k % ST_DEPTH, s = ST_DEPTH * g + kd, lap = (k / ST_DEPTH) & 1;
+      const uint32_t st = stg_g + kd * C::STAGE_BYTES;
       mbar_wait(bar0 + 8 * s, (uint32_t)lap, 1000u);
-      const SubMeta* mp = reinterpret_cast<const SubMeta*>(reinterpret_cast<const unsigned char*>(meta_g) + (k & 1) * C::STAGE_BYTES);
+      const SubMeta* mp = reinterpret_cast<const SubMeta*>(reinterpret_cast<const unsigned char*>(meta_g) + kd * C::STAGE_BYTES);
       const int Y = mp->Y, chunkG = mp->C0 + chunk;
       uint8_t* gpa = reinterpret_cast<uint8_t*>(mp->pa) + goffa;
       uint8_t* gpb = reinterpret_cast<uint8_t*>(mp->pb) + goffb;
