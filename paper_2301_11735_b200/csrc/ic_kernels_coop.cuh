@@ -7,15 +7,18 @@
 //   * the lattice stays in global memory (L2-resident: 1 MiB at most); the class tables and the per-lane move descriptors
 //     of the staged kernels sit in shared memory for the whole launch (no table fill per phase);
 //   * an item is FOUR coupled pairs (one 32-bit word of a 16-site plane vector, one Philox block): 65 536 items per phase at
-//     L = 1024 for 148 x 512 threads, so every thread has at most one short item per phase and the phase is one memory
-//     latency + one Philox block + one pairs4 (the item code of the staged kernels) long.  The four lanes of a quad load
-//     the same vectors (shifts and the FAR lane permutation work on whole vectors) and keep their own word;
+//     L = 1024 for 148 x 448 item threads, so every thread has at most one short item per phase and the phase is one memory
+//     latency + one Philox block + one pairs4 (the item code of the staged kernels) long;
 //   * the two phases of a sweep are separated by a barrier over the blocks of the replica (a counter in global memory:
-//     red.add + ld.acquire poll); the schedule of every sweep is derived on the device (the Philox call the host makes);
-//   * observables: per-thread sums -> warp REDUX -> block -> int64 atomics into a per-sweep accumulator that is double
-//     buffered by the sweep's parity; thread 0 of the replica's first block folds it after the sweep's second barrier
-//     (U5, the operations of k_fold in the same order) while the other blocks are already in the next sweep.
-// grid = (blocks per replica, replicas), replicas <= number of SMs; cooperative launch (all blocks co-resident).
+//     red.release + ld.acquire poll);
+//   * every block carries one service warp besides its item threads: while those are in phase 0 of sweep s it derives the
+//     schedule of sweep s+1 (the Philox call the host makes) and adds the block's sums of sweep s-1 (per-thread sums -> warp
+//     REDUX -> shared memory) into an accumulator in the workspace that is double buffered by the sweep's parity; the
+//     service warp of the replica's first block folds sweep s-1 (U5, the operations of k_fold in the same order) during
+//     phase 1.  Nothing serial is left on the item threads' path: two barriers per sweep.
+// grid = (blocks per replica, rows); a row of blocks takes the replicas row, row + rows, ... in turn (rows = min(replicas,
+// number of SMs)); cooperative launch (all blocks co-resident).  k_resvec_sweeps (below) runs the same items on a lattice
+// resident in shared memory, one block per replica, for 16 <= L <= 64.
 #pragma once
 #include "ic_common.cuh"
 #include "ic_kernels_ref.cuh"
