@@ -255,28 +255,15 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
   // Programmatic dependent launch: the next kernel of the stream may start its blocks as soon as ours leave their SMs;
   // it fills its tables (which no kernel writes) and then waits for the whole of this grid before touching the lattice.
   asm volatile("griddepcontrol.launch_dependents;");
-  {
-    const uint2* src = A.thr + (long long)r * THR_STRIDE;
-    uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
-    for (int k = tid; k < THR_STRIDE; k += ST_THREADS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
-    const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
-    uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
-    for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_THREADS) {
-      const int row = k >> 4, rr = row / 28, key = row - 28 * rr;   // keys with bit 2 set do not occur: null entries
-      uint2 d = __ldg(&dsrc[key * 8 + rr]);
-      d.y += smem0 + C::OFF_THR;                // low 16 bits: shared-memory address of the class base (< 64 KB)
-      desc_s[k] = d;
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(bar0 + 8 * s, 1);                                     // the producer warp (+ the bytes of its copies)
+      mbar_init(bar0 + 8 * (NST + s), ST_TPG / 32);                   // the warps of the consuming group
     }
-    if (tid == 0) {
-      for (int s = 0; s < NST; ++s) {
-        mbar_init(bar0 + 8 * s, 1);                                     // the producer warp (+ the bytes of its copies)
-        mbar_init(bar0 + 8 * (NST + s), ST_TPG / 32);                   // the warps of the consuming group
-      }
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  asm volatile("griddepcontrol.wait;" ::: "memory");                    // the previous phase / fold kernel is complete
   __syncthreads();
+  // From here the producers run ahead: their first bulk copies are in flight while the consumers fill the tables.
 
   const int lw = A.logL - 2, W = 1 << lw, Wm = W - 1;
   const int lognseg = lw - LOGSEG, nseg = 1 << lognseg;
@@ -303,6 +290,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
 
   if (warp >= ST_CONS / 32) {
     // ============================== producer warp g: both regions of every task of consumer group g =====================
+    asm volatile("griddepcontrol.wait;" ::: "memory");                  // the previous phase / fold kernel is complete
     const int g = warp - ST_CONS / 32;
     const int kyr = (lane >> 2) - 1, kx = lane & 3;                     // lane = staged row (ky_rel + 1) * 4 + kx
     const int hf = lane < C::ROWS ? halo_flags(TYPE, A.phase, A.p2, kyr, kx) : 0;
@@ -393,6 +381,23 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     // =========================================== consumer warps ====================================================
     // item = one 16-byte vector of a-sites (b-sites for NEAR-H) = 16 coupled pairs: sub-task (U, half), plane/row selector
     // hi, chunk of 16 plane columns (SEG / 16 = 32 chunks = the lanes of a warp); all but the chunk are uniform in a warp
+    {
+      // class tables of the replica and the per-lane move descriptors of the sweep type (written by no kernel: this overlaps
+      // the tail of the previous launch where two blocks fit an SM, and the producers' first copies everywhere)
+      const uint2* src = A.thr + (long long)r * THR_STRIDE;
+      uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
+      for (int k = tid; k < THR_STRIDE; k += ST_CONS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
+      const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
+      uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
+      for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_CONS) {
+        const int row = k >> 4, rr = row / 28, key = row - 28 * rr;   // keys with bit 2 set do not occur: null entries
+        uint2 d = __ldg(&dsrc[key * 8 + rr]);
+        d.y += smem0 + C::OFF_THR;                // low 16 bits: shared-memory address of the class base (< 64 KB)
+        desc_s[k] = d;
+      }
+      asm volatile("griddepcontrol.wait;" ::: "memory");                // before the first store to the lattice
+      asm volatile("bar.sync 1, %0;" ::"n"(ST_CONS) : "memory");        // the consumers' tables are complete
+    }
     const int g = warp >> 3, wg = warp & 7, sub = wg >> 1, hi = wg & 1, chunk = lane, U = sub >> 1, half = sub & 1, X0 = chunk << 4;
     const uint32_t s_desc = smem0 + C::OFF_DESC + (uint32_t)(lane & 15) * 8u;
     const uint32_t cb = ((uint32_t)r | (TAG_UPDATE << 28)) ^ A.rk[1];
