@@ -31,7 +31,7 @@ struct ic_ctx {
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; CoopScratch* d_coop; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; CoopScratch* d_coop; unsigned int* d_task_ctr; int8_t* d_stage;
   // host (pinned)
   uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
@@ -80,6 +80,7 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   b += align256((size_t)replicas * sizeof(ReplicaObs));            // integers and sums
   b += 256;                                                        // scratch for ic_debug_recompute
   b += align256((size_t)replicas * sizeof(CoopScratch));           // per-sweep sums and barrier counters of the one-launch kernel
+  b += align256((size_t)replicas * TASK_CTR_STRIDE * 4);           // task counters of the staged kernels
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
   return b;
 }
@@ -302,6 +303,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   c->d_obs = (ReplicaObs*)p; p += align256((size_t)replicas * sizeof(ReplicaObs));
   c->d_scratch8 = (long long*)p; p += 256;
   c->d_coop = (CoopScratch*)p; p += align256((size_t)replicas * sizeof(CoopScratch));
+  c->d_task_ctr = (unsigned int*)p; p += align256((size_t)replicas * TASK_CTR_STRIDE * 4);
   c->d_stage = (int8_t*)p;
   c->h_thr = nullptr; c->h_obs = nullptr; c->thr_copied = nullptr;
 
@@ -311,6 +313,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   if (cudaEventCreateWithFlags(&c->thr_copied, cudaEventDisableTiming) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaEventCreate"));
   memset(c->h_thr, 0, (size_t)replicas * THR_STRIDE * sizeof(uint2));
   cudaError_t e = cudaMemsetAsync(c->d_obs, 0, (size_t)replicas * sizeof(ReplicaObs), c->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->d_task_ctr, 0, (size_t)replicas * TASK_CTR_STRIDE * 4, c->stream);
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaMemsetAsync(observables)"));
   {
     std::vector<uint2> desc(2 * DESC_ENTRIES);
@@ -618,7 +621,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     a.type = par[0]; a.p1 = par[1]; a.p2 = par[2];
     bool absolute = false;
     for (int phase = 0; phase < 2; ++phase) {
-      a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase);
+      a.phase = phase; a.c2 = (uint32_t)(2 * c->sweep + (uint64_t)phase); a.task_ctr = c->d_task_ctr + phase;
       const bool staged = staged_ok(c) && (c->variant == 3 || c->variant == 0);
       const bool tiled = tiled_ok(c) && (c->variant == 0 || c->variant == 2);
       absolute = staged;     // the staged kernels report M, Ms of the updated sites instead of their changes
@@ -627,7 +630,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     }
     {
       long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * s : nullptr;
-      IC_CUDA(launch_pdl(k_fold, dim3((unsigned)((c->replicas + 127) / 128)), dim3(128), 0, c->stream, c->d_obs, c->replicas, c->delta, c->V, qJ, trow, absolute ? 1 : 0));
+      IC_CUDA(launch_pdl(k_fold, dim3((unsigned)((c->replicas + 127) / 128)), dim3(128), 0, c->stream, c->d_obs, c->replicas, c->delta, c->V, qJ, trow, absolute ? 1 : 0, c->d_task_ctr));
     }
     c->launches++;
     IC_CUDA(cudaGetLastError());
@@ -733,7 +736,7 @@ extern "C" int ic_sweep_maps(ic_ctx* c, const double* h_T, int64_t nmaps, int64_
     else if (c->layout == LAY_P2) k_map_update<LAY_P2><<<grid, 256, 0, c->stream>>>(a);
     else k_map_update<LAY_P16><<<grid, 256, 0, c->stream>>>(a);
     long long* trow = d_trace ? (long long*)d_trace + 6LL * c->replicas * m : nullptr;
-    k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ, trow, 0);
+    k_fold<<<(c->replicas + 127) / 128, 128, 0, c->stream>>>(c->d_obs, c->replicas, c->delta, c->V, qJ, trow, 0, (unsigned int*)nullptr);
     c->launches += 4;
     IC_CUDA(cudaGetLastError());
     c->sweep += 1;

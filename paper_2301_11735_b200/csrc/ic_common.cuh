@@ -158,6 +158,10 @@ struct ReplicaObs {
 };
 static_assert(sizeof(ReplicaObs) == 144, "ReplicaObs layout");
 
+// Task counters of the staged kernels: TASK_CTR_STRIDE words per replica (a cache line of its own), word p = phase p of the
+// sweep in progress; zeroed by ic_create and by k_fold after every sweep.
+constexpr int TASK_CTR_STRIDE = 32;
+
 // Parameters of one phase of one sweep (schedule S1, U4), the same for all replicas
 // (precedent: identical maps for all lattice copies).
 struct PhaseArgs {
@@ -166,6 +170,7 @@ struct PhaseArgs {
   const uint2* desc;             // move descriptors of this sweep type (tiled kernels), [28*8]
   const uint2* desc32;           // move descriptors (coefficients, info) of both sweep types (staged kernels), [2][256]
   ReplicaObs* obs;               // [replicas]
+  unsigned int* task_ctr;        // staged kernels: task counter of this phase, one per replica (stride TASK_CTR_STRIDE)
   long long lat_stride;          // bytes per replica
   int L, logL;
   int type;                      // 0 FAR (partner = (x^mx, y^my)), 1 NEAR (dominoes)

@@ -153,12 +153,14 @@ __global__ void __launch_bounds__(256) k_ref_phase(PhaseArgs A) {
 
 // U5: after a sweep, E = Delta*n2 + V*bV + (J/4)*bJ and the running sums, one thread per
 // replica, IEEE fp64 with one rounding per operation (no FMA contraction: explicit _rn intrinsics).
-__global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row, int absolute) {
+__global__ void k_fold(ReplicaObs* obs, int replicas, double delta, double V, double quarterJ, long long* trace_row, int absolute,
+                       unsigned int* task_ctr) {
   asm volatile("griddepcontrol.launch_dependents;");   // no-ops unless launched as a programmatic dependent (staged path)
   asm volatile("griddepcontrol.wait;" ::: "memory");
   int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= replicas) return;
   ReplicaObs* o = &obs[r];
+  if (task_ctr) { task_ctr[TASK_CTR_STRIDE * r] = 0u; task_ctr[TASK_CTR_STRIDE * r + 1] = 0u; }   // both phases are complete: the staged kernels' task counters
   if (absolute) { o->M = o->Mnext; o->Ms = o->Msnext; o->Mnext = 0; o->Msnext = 0; }   // the two phases covered every site once
   const double E = __dadd_rn(__dadd_rn(__dmul_rn(delta, (double)o->n2), __dmul_rn(V, (double)o->bV)),
                              __dmul_rn(quarterJ, (double)o->bJ));

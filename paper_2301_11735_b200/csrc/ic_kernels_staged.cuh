@@ -314,16 +314,37 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       }
     };
     uint32_t hl[2], hr[2];
+    // The first 15/16 of the tasks are dealt statically (task b + g G + k 2G to group g of block b of G); the rest is handed
+    // out by a counter of the replica in global memory (zeroed by k_fold after every sweep): whichever producer is ready
+    // takes the next one, so the blocks of a launch -- and the two groups of a block -- finish within one task of each
+    // other whatever the speed of their SMs (with all tasks dealt statically the SMs idle for 4 % of a launch; with all
+    // tasks from the counter its one address limits the launch: about 190 atomics per microsecond).  The next task is asked
+    // for one task ahead and looked at after the current stage is handed over.
+    unsigned int* ctr = A.task_ctr + TASK_CTR_STRIDE * r;
     const int tstep = ST_GROUPS * (int)gridDim.x;
-    halo_load((int)blockIdx.x + g * (int)gridDim.x, hl, hr);
-    for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += tstep, ++k) {
+    const int T0 = ((ntasks - (ntasks >> 4)) / tstep) * tstep;          // static part: the same number of tasks for every producer
+    int t = (int)blockIdx.x + g * (int)gridDim.x;
+    if (t >= T0) {
+      int tt = 0;
+      if (lane == 0) tt = T0 + (int)atomicAdd(ctr, 1u);
+      t = __shfl_sync(0xFFFFFFFFu, tt, 0);
+    }
+    halo_load(t, hl, hr);
+    for (int k = 0;; ++k) {
       const int kd = k % ST_DEPTH, s = ST_DEPTH * g + kd, lap = (k / ST_DEPTH) & 1;
       const uint32_t full = bar0 + 8 * s;
+      mbar_wait(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1), 20000u);
+      unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
+      if (t >= ntasks) {
+        // no task left: the group learns it from the task records (Y = -1) of one more, empty stage
+        if (lane >= 28) (reinterpret_cast<SubMeta*>(stg + C::OFF_SMETA) + (lane - 28))->Y = -1;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(full);
+        break;
+      }
       int Yq[2], sg[2];
 #pragma unroll
       for (int U = 0; U < 2; ++U) { const int rho = region_of(t, U); Yq[U] = rho >> lognseg; sg[U] = rho & (nseg - 1); }
-      mbar_wait(bar0 + 8 * (NST + s), (uint32_t)(lap ^ 1), 20000u);
-      unsigned char* stg = smem + C::OFF_STAGE + s * C::STAGE_BYTES;
       if (lane == 0) {
         mbar_expect_tx(full, 2u * (uint32_t)C::REGION_BYTES);
 #pragma unroll
@@ -341,6 +362,8 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
           }
         }
       }
+      int tn_raw = t + tstep;                            // the next task: asked for now, looked at after the stage is handed over
+      if (tn_raw >= T0 && lane == 0) tn_raw = T0 + (int)atomicAdd(ctr, 1u);
       if (lane >= 28) {
         // sub-task (U, half): where its items store to, and the coordinates for the Philox counters
         const int sub = lane - 28, U = sub >> 1, half = sub & 1, Y = Yq[U], seg = sg[U];
@@ -373,9 +396,10 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
           if (hf & 2) reinterpret_cast<uint32_t*>(stg + C::OFF_HALO)[U * 64 + 32 + lane] = hr[U];
         }
       }
-      halo_load(t + tstep, hl, hr);
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
+      t = __shfl_sync(0xFFFFFFFFu, tn_raw, 0);
+      halo_load(t, hl, hr);
     }
   } else {
     // =========================================== consumer warps ====================================================
@@ -461,12 +485,13 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
     const uint32_t stg_g = smem0 + C::OFF_STAGE + ST_DEPTH * g * C::STAGE_BYTES;
     const SubMeta* meta_g = reinterpret_cast<const SubMeta*>(smem + C::OFF_STAGE + ST_DEPTH * g * C::STAGE_BYTES + C::OFF_SMETA) + sub;
 
-    for (int t = blockIdx.x + g * gridDim.x, k = 0; t < ntasks; t += ST_GROUPS * gridDim.x, ++k) {
+    for (int k = 0;; ++k) {
       const int kd = k % ST_DEPTH, s = ST_DEPTH * g + kd, lap = (k / ST_DEPTH) & 1;
       const uint32_t st = stg_g + kd * C::STAGE_BYTES;
       mbar_wait(bar0 + 8 * s, (uint32_t)lap, 1000u);
       const SubMeta* mp = reinterpret_cast<const SubMeta*>(reinterpret_cast<const unsigned char*>(meta_g) + kd * C::STAGE_BYTES);
       const int Y = mp->Y, chunkG = mp->C0 + chunk;
+      if (Y < 0) break;                                                 // the producer found no task left
       uint8_t* gpa = reinterpret_cast<uint8_t*>(mp->pa) + goffa;
       uint8_t* gpb = reinterpret_cast<uint8_t*>(mp->pb) + goffb;
       uint8_t* gpl = nullptr;
