@@ -410,14 +410,24 @@ __global__ void __launch_bounds__(ST_THREADS, 1) k_staged_phase(const __grid_con
       // the tail of the previous launch where two blocks fit an SM, and the producers' first copies everywhere)
       const uint2* src = A.thr + (long long)r * THR_STRIDE;
       uint32_t* thr_s = reinterpret_cast<uint32_t*>(smem + C::OFF_THR);
-      for (int k = tid; k < THR_STRIDE; k += ST_CONS) { const uint2 v = __ldg(&src[k]); thr_s[k] = v.x; thr_s[THR_STRIDE + k] = v.y; }
       const uint2* dsrc = A.desc32 + (TYPE == PH_FAR ? 0 : ST_DESC_ENTRIES);
       uint2* desc_s = reinterpret_cast<uint2*>(smem + C::OFF_DESC);
-      for (int k = tid; k < ST_DESC_SMEM / 8; k += ST_CONS) {
-        const int row = k >> 4, rr = row / 28, key = row - 28 * rr;   // keys with bit 2 set do not occur: null entries
-        uint2 d = __ldg(&dsrc[key * 8 + rr]);
-        d.y += smem0 + C::OFF_THR;                // low 16 bits: shared-memory address of the class base (< 64 KB)
-        desc_s[k] = d;
+      // all loads of a thread are issued before its first store: one memory latency for the fill, not one per entry
+      constexpr int NT = (THR_STRIDE + ST_CONS - 1) / ST_CONS, ND = (ST_DESC_SMEM / 8 + ST_CONS - 1) / ST_CONS;
+      uint2 tv[NT], dv[ND];
+#pragma unroll
+      for (int i = 0; i < NT; ++i) { const int k = tid + i * ST_CONS; tv[i] = k < THR_STRIDE ? __ldg(&src[k]) : make_uint2(0u, 0u); }
+#pragma unroll
+      for (int i = 0; i < ND; ++i) {
+        const int k = tid + i * ST_CONS, row = k >> 4, rr = row / 28, key = row - 28 * rr;   // keys with bit 2 set do not occur: null entries
+        dv[i] = k < ST_DESC_SMEM / 8 ? __ldg(&dsrc[key * 8 + rr]) : make_uint2(0u, 0u);
+      }
+#pragma unroll
+      for (int i = 0; i < NT; ++i) { const int k = tid + i * ST_CONS; if (k < THR_STRIDE) { thr_s[k] = tv[i].x; thr_s[THR_STRIDE + k] = tv[i].y; } }
+#pragma unroll
+      for (int i = 0; i < ND; ++i) {
+        const int k = tid + i * ST_CONS;
+        if (k < ST_DESC_SMEM / 8) { dv[i].y += smem0 + C::OFF_THR; desc_s[k] = dv[i]; }   // low 16 bits: shared-memory address of the class base (< 64 KB)
       }
       asm volatile("griddepcontrol.wait;" ::: "memory");                // before the first store to the lattice
       asm volatile("bar.sync 1, %0;" ::"n"(ST_CONS) : "memory");        // the consumers' tables are complete
