@@ -49,7 +49,9 @@ enum {
   IC_ERR_PARAM = -3,     /* |n| > 1, NaN/inf parameter, T <= 0, nsweeps < 0, sweep counter >= 2^31     */
   IC_ERR_WORKSPACE = -4, /* workspace NULL, smaller than ic_workspace_bytes(), or not 256-B aligned   */
   IC_ERR_CHARGE = -5,    /* ic_set_state: a code outside 0..3 or sum S != Q; ic_init_charges: bad counts */
-  IC_ERR_CUDA = -6       /* a CUDA call failed; ic_strerror(IC_ERR_CUDA) returns its message          */
+  IC_ERR_CUDA = -6,      /* a CUDA call failed; ic_strerror(IC_ERR_CUDA) returns its message          */
+  IC_ERR_STATIC_MAX = -7 /* ic_largest_cluster_static only: L > IC_STATIC_CLUSTER_MAX_L, the lattice does not
+                            fit the scratch array built into the library                              */
 };
 
 /* Filled by ic_observables, one per replica (host memory, caller-owned).
@@ -148,6 +150,37 @@ int ic_sweep_maps(ic_ctx* ctx, const double* h_T, int64_t nmaps, int64_t K, void
 size_t ic_cluster_scratch_bytes(int L);
 int ic_largest_cluster(ic_ctx* ctx, int replica, int which, void* d_scratch, size_t scratch_bytes, int64_t* h_out2);
 int ic_snapshot_ppm(ic_ctx* ctx, int replica, const char* path);
+
+/* ---- the same cluster count for callers that have no device memory to give -------------------------------------------
+ * ic_largest_cluster needs 8 bytes of device scratch per site (union-find parents and cluster sizes) and every other
+ * call of this library needs a workspace, all of it allocated by the caller.  Some callers cannot allocate when they want
+ * the size of the drop: an analysis hook that runs inside another program's time step after that
+ * program has handed the whole HBM to its own pool; a plug-in whose host forbids cudaMalloc / cudaFree in its steady
+ * state because both wait for the whole device and stall every other stream; a monitor that must stay inside a fixed
+ * memory budget.  For them this ONE entry point works without a context, a workspace or a scratch argument: its scratch is
+ * an array compiled into the library (8 MiB of device memory per GPU, held by every GPU that loads the library from the
+ * first CUDA call of the process on that GPU until the process exits, whether or not this call is ever made).
+ *
+ *   d_codes   DEVICE, L*L public site codes (0..3 as in ic_set_state / ic_state; one byte per site, row-major), read only;
+ *             codes are taken modulo 4.  L a power of two, 4 <= L <= IC_STATIC_CLUSTER_MAX_L.
+ *   which     0: sites with S != 0, 1: S = +1, 2: S = -1 (as in ic_largest_cluster; 4-neighbour, periodic).
+ *   d_out2    DEVICE, two int64 written by the call: (size of the largest cluster, number of clusters).
+ *   stream    a cudaStream_t (NULL = default stream) of the calling thread's CURRENT device; d_codes and d_out2 must be
+ *             memory of that device.  The call only enqueues four kernels and returns; synchronise the stream (or order
+ *             later work on it) before reading d_out2.  Both buffers stay owned by the caller.
+ *
+ * It calls no cudaMalloc, cudaFree or any library routine that allocates.  The first call on each device (with that
+ * device current) looks up the device address of the built-in array with cudaGetSymbolAddress and keeps it; make that
+ * first call at start-up, before any stream capture begins in the process.  Later calls only launch.
+ * All calls on one GPU share the one array, and it keeps what the previous call left there: every call rewrites the part
+ * it uses before reading it (nothing has to be cleared by the caller), but two calls whose kernels can overlap on the
+ * GPU -- different streams, different host threads, different contexts of one process -- race on it and give garbage.
+ * Put them on one stream or order them with events.
+ * Errors (nothing is launched): IC_ERR_NULL (d_codes or d_out2 NULL), IC_ERR_SIZE (L < 4 or not a power of two),
+ * IC_ERR_STATIC_MAX (L > IC_STATIC_CLUSTER_MAX_L: the lattice does not fit the built-in array; use ic_largest_cluster
+ * with scratch of your own), IC_ERR_PARAM (which outside 0..2), IC_ERR_CUDA.                                              */
+#define IC_STATIC_CLUSTER_MAX_L 1024
+int ic_largest_cluster_static(const int8_t* d_codes, int L, int which, int64_t* d_out2, void* cuda_stream);
 
 /* Kernel selection: 0 = automatic (default), 1 = reference kernels (one thread per pair, global memory),
  * 2 = tiled kernels (8 bits/site, 64 <= L <= 2048: vectors loaded straight from global memory), 3 = staged kernels

@@ -12,7 +12,9 @@ import numpy as np
 from . import build as _build
 
 IC_OK, IC_ERR_NULL, IC_ERR_SIZE, IC_ERR_PARAM, IC_ERR_WORKSPACE, IC_ERR_CHARGE, IC_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
+IC_ERR_STATIC_MAX = -7
 IC_N_CLASSES = 3267
+IC_STATIC_CLUSTER_MAX_L = 1024
 
 
 class ic_obs(C.Structure):
@@ -42,6 +44,7 @@ EXPORTS = {
     "ic_cluster_scratch_bytes": (C.c_size_t, [C.c_int]),
     "ic_largest_cluster": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.POINTER(C.c_int64)]),
     "ic_snapshot_ppm": (C.c_int, [C.c_void_p, C.c_int, C.c_char_p]),
+    "ic_largest_cluster_static": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
     "ic_sweep_count": (C.c_int64, [C.c_void_p]),
     "ic_charge": (C.c_int64, [C.c_void_p]),
     "ic_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
@@ -73,6 +76,28 @@ class IcError(RuntimeError):
 def _check(code, where):
     if code != IC_OK:
         raise IcError(code, where)
+
+
+def largest_cluster_static(d_codes, which, d_out2, stream=None):
+    """ic_largest_cluster_static: (largest cluster, number of clusters) of one lattice, without a Sim, a workspace or scratch.
+
+    For code that cannot allocate device memory when it wants the answer (a hook inside a program that gave all of HBM to its
+    own pool, a host that forbids cudaMalloc / cudaFree because they stall the device, a fixed memory budget): the scratch
+    is an 8 MiB array built into the library, one per GPU, shared by all calls, so L <= IC_STATIC_CLUSTER_MAX_L (1024) and
+    calls that overlap on the GPU race.  Nothing is allocated here either: the caller passes both tensors.
+
+    d_codes: CUDA int8 tensor [L, L] of public site codes; d_out2: CUDA int64 tensor of 2 elements on the same device, written
+    asynchronously on `stream` (default: torch's current stream of that device); read it after the stream has caught up.
+    """
+    import torch
+    assert d_codes.is_cuda and d_codes.is_contiguous() and d_codes.element_size() == 1 and d_codes.dim() == 2
+    assert d_out2.is_cuda and d_out2.dtype == torch.int64 and d_out2.numel() == 2 and d_out2.is_contiguous()
+    assert d_out2.device == d_codes.device and d_codes.shape[0] == d_codes.shape[1]
+    with torch.cuda.device(d_codes.device):              # the entry point works on the current device
+        st = torch.cuda.current_stream() if stream is None else stream
+        _check(lib.ic_largest_cluster_static(C.c_void_p(d_codes.data_ptr()), int(d_codes.shape[0]), int(which),
+                                             C.c_void_p(d_out2.data_ptr()), C.c_void_p(st.cuda_stream)), "ic_largest_cluster_static")
+    return d_out2
 
 
 class Sim:

@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <thread>
 #include <vector>
@@ -796,6 +797,79 @@ extern "C" int ic_snapshot_ppm(ic_ctx* c, int replica, const char* path) {
   return IC_OK;
 }
 
+// ---- ic_largest_cluster_static: the cluster count without a context, a workspace or a scratch argument ---------------------
+// For callers that cannot get device memory when they need the answer (see include/ic.h: a hook inside a program that gave
+// the whole HBM to its own pool, a host that forbids cudaMalloc / cudaFree because they wait for the whole device, a fixed
+// memory budget).  The union-find needs parent[N] and size[N]; here both live in an array that is part of the library's
+// device image: 2 x 1024 x 1024 ints = 8 MiB on every GPU that loads the library, until the process exits.
+// One array per GPU, shared by every call: a call rewrites parent[0..N) and size[0..N) (k_ccs_init) before any kernel
+// reads them, so what the previous call left behind does not matter; calls that overlap on the GPU race on it.
+constexpr int CCS_MAX_L = IC_STATIC_CLUSTER_MAX_L;
+constexpr long long CCS_MAX_N = (long long)CCS_MAX_L * CCS_MAX_L;
+static __device__ __align__(256) int g_ccs_scratch[2 * CCS_MAX_N];
+// On the host, `g_ccs_scratch` is NOT the device address: it is the host-side shadow variable the runtime uses as a handle.
+// A kernel handed `g_ccs_scratch` from host code would write through a host address (a fault, or on systems where the GPU
+// reaches host memory, silent corruption of something else).  The device address is asked for once per device, below.
+constexpr int CCS_MAX_DEVICES = 64;
+struct CcsDevice { int* scratch; int sm_count; };
+static CcsDevice g_ccs_dev[CCS_MAX_DEVICES] = {};
+static std::mutex g_ccs_mutex;
+
+// Set-up for the calling thread's current device: device address of the array and the SM count.  Called by every
+// ic_largest_cluster_static; only the first call per device talks to the runtime.  No allocation.
+static int ccs_setup(CcsDevice* out) {
+  int dev = -1;
+  IC_CUDA(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_ccs_mutex);
+  const bool cached = dev >= 0 && dev < CCS_MAX_DEVICES;
+  if (cached && g_ccs_dev[dev].scratch) { *out = g_ccs_dev[dev]; return IC_OK; }
+  CcsDevice d{nullptr, 0};
+  IC_CUDA(cudaGetSymbolAddress((void**)&d.scratch, g_ccs_scratch));   // the copy of the array on the CURRENT device
+  IC_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+  if (!d.scratch || ((uintptr_t)d.scratch & 255) != 0 || d.sm_count < 1) return cuda_fail(cudaErrorInvalidSymbol, "address of the built-in scratch array");
+  if (cached) g_ccs_dev[dev] = d;
+  *out = d;
+  return IC_OK;
+}
+
+// parent[i] = i for sites inside the selection, -1 outside; size[i] = 0; the caller's two outputs start at zero.
+// Everything the later kernels read is written here first: the array still holds the previous call's forest.
+__global__ void k_ccs_init(const int8_t* __restrict__ codes, int N, int which, int* __restrict__ parent, int* __restrict__ size,
+                           long long* __restrict__ out2) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) { out2[0] = 0; out2[1] = 0; }
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+    parent[i] = cc_inside(codes[i] & 3, which) ? i : -1;
+    size[i] = 0;
+  }
+}
+
+static bool ccs_gpu_can_read(const void* p) {      // false for ordinary (pageable, unregistered) host memory
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type != cudaMemoryTypeUnregistered;
+}
+
+extern "C" int ic_largest_cluster_static(const int8_t* d_codes, int L, int which, int64_t* d_out2, void* cuda_stream) {
+  if (!d_codes || !d_out2) return IC_ERR_NULL;
+  if (L < 4 || (L & (L - 1)) != 0) return IC_ERR_SIZE;
+  if (L > CCS_MAX_L) return IC_ERR_STATIC_MAX;
+  if (which < 0 || which > 2) return IC_ERR_PARAM;
+  if (!ccs_gpu_can_read(d_codes) || !ccs_gpu_can_read(d_out2)) return IC_ERR_PARAM;
+  CcsDevice d;
+  { int rc = ccs_setup(&d); if (rc != IC_OK) return rc; }
+  const int N = L * L;
+  int logL = 0; while ((1 << logL) < L) ++logL;
+  int* parent = d.scratch; int* size = d.scratch + N;      // the first 8 N bytes of the array, whatever CCS_MAX_N is
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  const int nb = (int)std::min<long long>((N + 255) / 256, (long long)d.sm_count * 8);
+  k_ccs_init<<<nb, 256, 0, stream>>>(d_codes, N, which, parent, size, (long long*)d_out2);
+  k_cc_link<<<nb, 256, 0, stream>>>(L, logL, parent);
+  k_cc_count<<<nb, 256, 0, stream>>>(N, parent, size);
+  k_cc_max<<<nb, 256, 0, stream>>>(N, size, (long long*)d_out2);
+  IC_CUDA(cudaGetLastError());
+  return IC_OK;
+}
+
 extern "C" int ic_thresholds(ic_ctx* c, double T, uint32_t* h_out) {
   if (!c || !h_out) return IC_ERR_NULL;
   if (!(T > 0.0) || !std::isfinite(T)) return IC_ERR_PARAM;
@@ -844,6 +918,7 @@ extern "C" const char* ic_strerror(int code) {
     case IC_ERR_WORKSPACE: return "workspace is NULL, too small (see ic_workspace_bytes) or not 256-byte aligned";
     case IC_ERR_CHARGE: return "state rejected: a code outside 0..3 or sum S != Q";
     case IC_ERR_CUDA: return g_cuda_msg;
+    case IC_ERR_STATIC_MAX: return "ic_largest_cluster_static: L is larger than IC_STATIC_CLUSTER_MAX_L (1024), the lattice does not fit the scratch array built into the library; use ic_largest_cluster with scratch memory of your own";
     default: return "unknown error code";
   }
 }

@@ -56,7 +56,7 @@ def test_workspace_bytes_and_size_errors(pkg):
     assert lib.ic_create(C.byref(h), 64, 0.1, 0, 0, 0, 1, 1, 8, C.c_void_p(256), 16, None) == pkg.IC_ERR_WORKSPACE
     assert lib.ic_create(C.byref(h), 64, 0.1, 0, 0, 0, 1, 1, 8, C.c_void_p(257), 1 << 30, None) == pkg.IC_ERR_WORKSPACE
     assert h.value is None
-    for code in range(0, -7, -1):
+    for code in range(0, -8, -1):
         assert len(lib.ic_strerror(code)) > 0
     assert lib.ic_sweep(None, None, 1) == pkg.IC_ERR_NULL
     assert lib.ic_sweep_count(None) == -1
