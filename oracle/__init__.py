@@ -42,6 +42,8 @@ def lib():
         stp = C.POINTER(OrcState)
         L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]; L.orc_philox4x32_10.restype = None
         L.orc_philox4x32.argtypes = [u32p, u32p, C.c_int, u32p]; L.orc_philox4x32.restype = None
+        L.orc_set_update_rounds.argtypes = [C.c_int]; L.orc_set_update_rounds.restype = C.c_int
+        L.orc_get_update_rounds.argtypes = []; L.orc_get_update_rounds.restype = C.c_int
         L.orc_threshold.argtypes = [C.c_double] * 3 + [C.c_int] * 3 + [C.c_double]; L.orc_threshold.restype = C.c_uint32
         L.orc_recompute.argtypes = [i8p, C.c_int, C.c_int, i64p]; L.orc_recompute.restype = None
         L.orc_pair_table.argtypes = [C.c_int, C.c_int, i8p]; L.orc_pair_table.restype = C.c_int
@@ -90,6 +92,15 @@ def philox4x32(ctr, key, rounds):
     out = np.zeros(4, dtype=np.uint32)
     lib().orc_philox4x32(_p(c, C.c_uint32), _p(k, C.c_uint32), int(rounds), _p(out, C.c_uint32))
     return out
+
+
+def set_update_rounds(rounds):
+    """Philox rounds of the update stream for the runs that follow (UPDATE_ROUNDS = 7 is the default and what the library
+    uses); returns the previous value.  For the 7-versus-10-round ensemble comparison only."""
+    old = lib().orc_get_update_rounds()
+    if lib().orc_set_update_rounds(int(rounds)) != 0:
+        raise ValueError("rounds must be in 1..16")
+    return old
 
 
 def threshold(delta, V, J, dn2, dV, dJ, T):

@@ -83,6 +83,17 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* tags 0..3 here; oracle/ic_variants.c uses 4..7 */
 enum { TAG_UPDATE = 0, TAG_SCHED = 1, TAG_INIT = 2, TAG_S0 = 3 };
 
+/* Rounds of the update stream: ORC_UPDATE_ROUNDS (7, what the library is built with) unless a test asks for another
+ * member of the family -- tests/test_oracle_pins.py compares the sampled <E> and C at 7 and at 10 rounds.  Set between
+ * runs only (the sweeps read it from several threads). */
+static int g_update_rounds = ORC_UPDATE_ROUNDS;
+int orc_set_update_rounds(int rounds) {
+  if (rounds < 1 || rounds > 16) return -1;
+  g_update_rounds = rounds;
+  return 0;
+}
+int orc_get_update_rounds(void) { return g_update_rounds; }
+
 void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2,
                        uint32_t replica, uint32_t tag, uint32_t out[4]) {
   uint32_t ctr[4] = {c0, c1, c2, (replica & 0x0FFFFFFFu) | (tag << 28)};
@@ -90,7 +101,7 @@ void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2,
   /* DESIGN.md G5: the update stream of schedule S1 (one block per four pair updates) is Philox4x32-7, the
    * seven-round member of the family (Salmon et al. report 7 rounds as the fewest that pass BigCrush, 10 as the
    * default with a safety margin); every other stream (schedule, stage 1, S0 and the variants) uses 10 rounds. */
-  orc_philox4x32(ctr, key, tag == TAG_UPDATE ? ORC_UPDATE_ROUNDS : 10, out);
+  orc_philox4x32(ctr, key, tag == TAG_UPDATE ? g_update_rounds : 10, out);
 }
 
 /* ------------------------------------------------------------------------- */

@@ -26,7 +26,11 @@ typedef struct {
   int64_t n_attempt, n_accept, n_null; /* statistics                            */
 } orc_state;
 
-#define ORC_UPDATE_ROUNDS 7 /* Philox rounds of the update stream (G5) */
+#ifndef ORC_UPDATE_ROUNDS
+#define ORC_UPDATE_ROUNDS 7 /* Philox rounds of the update stream (G5); the default of orc_set_update_rounds */
+#endif
+int orc_set_update_rounds(int rounds); /* 1..16; 0 on success.  Not to be called while a sweep runs. */
+int orc_get_update_rounds(void);
 void orc_philox4x32(const uint32_t ctr[4], const uint32_t key[2], int rounds, uint32_t out[4]);
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 void orc_philox_tagged(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t replica, uint32_t tag, uint32_t out[4]);

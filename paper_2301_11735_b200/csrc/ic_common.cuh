@@ -41,7 +41,13 @@ IC_HD u32x4 philox4x32(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // Schedule and stage-1 streams: the default ten rounds.  Update stream (one block per four pair updates, the hot path):
 // Philox4x32-7, the seven-round member of the family that Salmon et al. report as the fewest rounds passing BigCrush
 // (SURVEY 8(d) "RNG ladder", G5).
-constexpr int PHILOX_UPDATE_ROUNDS = 7;
+// Compile-time switch (the oracle's twin is orc_set_update_rounds): build with -DIC_PHILOX_UPDATE_ROUNDS=10 for the default
+// member of the family; every kernel, the staged kernels' precomputed round keys included, follows this constant.
+#ifndef IC_PHILOX_UPDATE_ROUNDS
+#define IC_PHILOX_UPDATE_ROUNDS 7
+#endif
+constexpr int PHILOX_UPDATE_ROUNDS = IC_PHILOX_UPDATE_ROUNDS;
+static_assert(PHILOX_UPDATE_ROUNDS >= 2 && PHILOX_UPDATE_ROUNDS <= 10, "the staged kernels precompute the first two rounds and ten round keys");
 IC_HD u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
   return philox4x32<10>(c0, c1, c2, c3, k0, k1);
 }

@@ -236,3 +236,61 @@ def test_init_state_exact_counts_and_determinism():
     c = oracle.init_state(64, 64, 1000, 0, 9)
     rows = (c == 2).sum(1)
     assert rows.min() > 2 and rows.max() < 40                                 # spread over the lattice, not clumped
+
+
+def test_init_state_is_uniform_over_sites_and_signs():
+    """Stage 1 (reading U0) draws the charged sites uniformly without replacement and deals the signs among
+    them at random: over 400 seeds on an 8 x 8 lattice with 10 S=+1 and 6 S=-1 sites, the number of times each site is charged
+    (expected 100) and is S=+1 (expected 62.5) pass a chi-square test with 63 degrees of freedom -- a selection that is off by
+    one (a site that can never be drawn, or drawn twice as often) fails it by a wide margin -- and the uncharged sites are
+    sigma=+1 half of the time."""
+    L, N, p, m, S = 8, 64, 10, 6, 400
+    K = p + m
+    charged = np.zeros(N); plus = np.zeros(N); up = 0
+    for seed in range(1000, 1000 + S):
+        c = oracle.init_state(L, L, p, m, seed).reshape(-1)
+        assert (c == 2).sum() == p and (c == 3).sum() == m
+        charged += c >= 2; plus += c == 2; up += int((c == 0).sum())
+    for cnt, k in ((charged, K), (plus, p)):
+        q = k / N
+        var = S * q * (1 - q)                  # per lattice a site is chosen with probability q; the seeds are independent
+        chi2 = ((cnt - S * q) ** 2).sum() / var * (N - 1) / N      # the N counts sum to S k exactly: N-1 degrees of freedom
+        assert 30.0 < chi2 < 110.0, chi2       # chi-square(63): mean 63, sd 11.2; both tails beyond 3 sd are rejected
+        assert cnt.min() > 0.5 * S * q and cnt.max() < 1.6 * S * q
+    n_unch = S * (N - K)
+    assert abs(up - 0.5 * n_unch) < 4 * math.sqrt(0.25 * n_unch)
+
+
+@pytest.mark.parametrize("L,nsweeps", [(16, 12000), (32, 5000)])
+def test_seven_round_update_stream_samples_the_same_ensemble_as_ten_rounds(L, nsweeps):
+    """Reading G5 runs the update stream on Philox4x32-7, the member of the family with the fewest rounds its authors report
+    as passing BigCrush.  Beyond the exact 4 x 4 ensemble of test_oracle_exact, this compares what the physics sees at larger
+    sizes: <E>/N, C and <n2> of schedule S1 near the specific-heat maximum, 8 independent seeds per round count; the means at 7
+    and at 10 rounds agree within 3.5 standard errors of their difference, and the 10-round runs leave the switch as found."""
+    delta, V, J, T, n = 0.2, 1.0, 1.0, 1.3, 0.1          # C(T) is largest around T = 1.3 for these parameters
+    N = L * L
+    Q = round(n * N)
+    res = {}
+    assert oracle.UPDATE_ROUNDS == 7
+    for rounds in (7, 10):
+        old = oracle.set_update_rounds(rounds)
+        try:
+            rows = []
+            for seed in range(8):
+                code = oracle.init_state(L, L, Q, 0, 500 + seed)
+                lat = oracle.Lattice(code, delta, V, J, 500 + seed)
+                lat.sweep_s1(T, nsweeps // 2)
+                lat.reset_observables()
+                lat.sweep_s1(T, nsweeps)
+                o = lat.observables(T)
+                rows.append((o["sumE"] / o["nmeas"] / N, o["C"], float(lat.st.n2) / N))
+            res[rounds] = np.array(rows)
+        finally:
+            assert oracle.set_update_rounds(old) == rounds
+    assert oracle.lib().orc_get_update_rounds() == 7
+    assert not np.array_equal(res[7], res[10])                    # the switch does something
+    for k, name in enumerate(("E/N", "C", "n2/N")):
+        a, b = res[7][:, k], res[10][:, k]
+        err = math.sqrt(a.var(ddof=1) / len(a) + b.var(ddof=1) / len(b))
+        assert abs(a.mean() - b.mean()) < 3.5 * err, (name, a.mean(), b.mean(), err)
+    assert 1.0 < res[7][:, 1].mean() < 6.0                       # a real specific heat, not a frozen lattice
