@@ -25,8 +25,9 @@
  *   - the constraint of eq. (2), sum_i S_i = Q = llround(n*N), holds after every pair update.
  *   - all launches and copies go to the CUDA stream given to ic_create.  ic_sweep is asynchronous;
  *     ic_set_state, ic_init_charges, ic_observables, ic_state, ic_debug_recompute, ic_largest_cluster and
- *     ic_snapshot_ppm synchronise that stream (ic_thresholds and ic_schedule are host-only).  Every call makes the
- *     device the context was created on current for the calling thread (and leaves it current).
+ *     ic_snapshot_ppm synchronise that stream (ic_thresholds and ic_schedule are host-only).  Every call that takes
+ *     a context and touches the device makes the device the context was created on current for the calling thread (and
+ *     leaves it current); ic_destroy and the host-only getters do not change the current device.
  *   - one context must not be used from two host threads at once.
  */
 #ifndef IC_H
@@ -108,6 +109,16 @@ int ic_sweep_trace(ic_ctx* ctx, const double* h_T, int64_t nsweeps, int64_t* d_t
 int ic_reset_observables(ic_ctx* ctx);            /* zeroes nmeas and the fp64 sums (not the lattice)  */
 int ic_observables(ic_ctx* ctx, ic_obs* h_out);   /* h_out[replicas], HOST; synchronises the stream    */
 int ic_state(ic_ctx* ctx, int replica, int8_t* h_codes_out); /* L*L public codes, HOST; synchronises   */
+
+/* Resume.  The lattices, the global sweep counter and the seed determine every later pair update (the random stream is
+ * keyed by (seed, replica, sweep, slot)); nmeas and the fp64 sums carry the averages of PAPER.md:49-53 across the break.
+ * To save a run: ic_state of every replica, ic_sweep_count, ic_observables.  To continue it: ic_create with the same L, n,
+ * Delta, V, J, seed, replicas (bits_per_site and the kernel variant are free), ic_set_state for every replica, then
+ * ic_restore(ctx, saved sweep count, saved ic_obs[replicas]): sets the sweep counter and, per replica, nmeas and the eight
+ * sums from h_in (HOST); the exact integers in h_in are ignored -- ic_set_state has recomputed them from the lattice.  The
+ * continued run is then bit-identical to the uninterrupted one (lattices, integers, sums).  Synchronises the stream.
+ * IC_ERR_PARAM: sweep_count outside [0, 2^31), nmeas < 0, a sum that is not finite.                                      */
+int ic_restore(ic_ctx* ctx, int64_t sweep_count, const ic_obs* h_in);
 
 /* Full recomputation of (n2,bV,bJ,M,Ms,Q) from the lattice by a device reduction, straight from eq. (3);
  * out6 is HOST memory.  Must equal the incrementally tracked integers at any time.                    */

@@ -36,6 +36,7 @@ EXPORTS = {
     "ic_reset_observables": (C.c_int, [C.c_void_p]),
     "ic_observables": (C.c_int, [C.c_void_p, C.POINTER(ic_obs)]),
     "ic_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "ic_restore": (C.c_int, [C.c_void_p, C.c_int64, C.POINTER(ic_obs)]),
     "ic_debug_recompute": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "ic_thresholds": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(C.c_uint32)]),
     "ic_schedule": (C.c_int, [C.c_void_p, C.c_uint64, C.POINTER(C.c_int32)]),
@@ -161,7 +162,9 @@ class Sim:
             raise IcError(IC_ERR_SIZE, "scratch size")
         buf = getattr(self, "_scratch_buf", None)
         if buf is None or buf.numel() < nbytes + 256:
-            with self.torch.cuda.device(self.device):
+            # allocated on the context's stream: the block the old buffer gives back may still be in use by kernels queued there,
+            # and the caching allocator only hands it out again to that same stream
+            with self.torch.cuda.device(self.device), self.torch.cuda.stream(self.stream):
                 self._scratch_buf = buf = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device=self.device)
         return (buf.data_ptr() + 255) & ~255
 
@@ -170,7 +173,10 @@ class Sim:
         arr, p = self._T(T)
         nbytes = lib.ic_maps_scratch_bytes(self.L, int(K))
         ptr = self._scratch(nbytes)
-        tr = self.torch.empty((int(nmaps), self.replicas, 6), dtype=self.torch.int64, device=self.device) if trace else None
+        tr = None
+        if trace:
+            with self.torch.cuda.device(self.device), self.torch.cuda.stream(self.stream):
+                tr = self.torch.empty((int(nmaps), self.replicas, 6), dtype=self.torch.int64, device=self.device)
         _check(lib.ic_sweep_maps(self.h, p, int(nmaps), int(K), C.c_void_p(ptr), nbytes,
                                  C.c_void_p(tr.data_ptr()) if trace else None), "ic_sweep_maps")
         return tr
@@ -193,6 +199,15 @@ class Sim:
         out = (ic_obs * self.replicas)()
         _check(lib.ic_observables(self.h, out), "ic_observables")
         return [{f: getattr(o, f) for f, _ in ic_obs._fields_} for o in out]
+
+    def restore(self, sweep_count, observables):
+        """ic_restore: continue a saved run -- `observables` is what observables() returned when the run was saved."""
+        arr = (ic_obs * self.replicas)()
+        assert len(observables) == self.replicas
+        for o, d in zip(arr, observables):
+            for f, _ in ic_obs._fields_:
+                setattr(o, f, d[f])
+        _check(lib.ic_restore(self.h, int(sweep_count), arr), "ic_restore")
 
     def state(self, replica=0, out=None):
         if out is None:

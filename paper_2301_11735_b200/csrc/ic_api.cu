@@ -5,6 +5,7 @@
 // on the host except stage 1 of the algorithm (the initial configuration with the prescribed
 // charge), which is a sequential selection and belongs to ic_create, not to the sweep.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -351,7 +352,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
 
 extern "C" int ic_destroy(ic_ctx* c) {
   if (!c) return IC_ERR_NULL;
-  if (c->stream || true) cudaStreamSynchronize(c->stream);
+  cudaStreamSynchronize(c->stream);
   if (c->h_thr) cudaFreeHost(c->h_thr);
   if (c->h_obs) cudaFreeHost(c->h_obs);
   if (c->thr_copied) cudaEventDestroy(c->thr_copied);
@@ -455,7 +456,7 @@ static int launch_phase_p16(ic_ctx* c, PhaseArgs a) {
 template <int TYPE, int CW, int BITS>
 static int launch_staged_bits(ic_ctx* c, const PhaseArgs& a, dim3 grid) {
   using C = StagedCfg<TYPE, BITS>;
-  static bool configured[64] = {};   // per instantiation and per device: the attribute belongs to the device's copy of the kernel
+  static std::atomic<bool> configured[64] = {};   // per instantiation and per device: the attribute belongs to the device's copy of the kernel
   if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
     IC_CUDA(cudaFuncSetAttribute(k_staged_phase<TYPE, CW, BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     if (c->device >= 0 && c->device < 64) configured[c->device] = true;
@@ -473,7 +474,7 @@ static bool coop_ok(const ic_ctx* c) {
 }
 template <int BITS>
 static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
-  static bool configured[64] = {};
+  static std::atomic<bool> configured[64] = {};
   if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
     IC_CUDA(cudaFuncSetAttribute(k_coop_sweeps<BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, COOP_SMEM_BYTES));
     if (c->device >= 0 && c->device < 64) configured[c->device] = true;
@@ -491,11 +492,21 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
   const int threads = 32 + (int)std::min<long long>(COOP_THREADS - 32, std::max<long long>(128, ((items + nblk - 1) / nblk + 31) / 32 * 32));
   dim3 grid((unsigned)nblk, (unsigned)rows);
   IC_CUDA(cudaMemsetAsync(c->d_coop, 0, (size_t)c->replicas * sizeof(CoopScratch), c->stream));
+  static_assert(COOP_BAR_BASE == 0xFFFFFFFFu, "the barrier counters are set bytewise");
+  IC_CUDA(cudaMemset2DAsync(&c->d_coop->arrived, sizeof(CoopScratch), 0xFF, sizeof(unsigned int), (size_t)c->replicas, c->stream));
   void* args[] = {(void*)&a};
-  const cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream);
-  if (e == cudaErrorCooperativeLaunchTooLarge) {   // fewer SMs available than the device reports (MPS, green contexts): per-phase kernels from now on
+  cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream);
+  // fewer SMs available than the device reports (MPS, green contexts): the results do not depend on the number of blocks
+  // per replica, so try again with half as many before giving the kernel up
+  while (e == cudaErrorCooperativeLaunchTooLarge && grid.x > 1) {
     (void)cudaGetLastError();
-    c->coop_supported = false;
+    grid.x = (grid.x + 1) / 2;
+    e = cudaLaunchCooperativeKernel((const void*)k_coop_sweeps<BITS>, grid, dim3(threads), args, (size_t)COOP_SMEM_BYTES, c->stream);
+  }
+  if (e == cudaErrorCooperativeLaunchTooLarge) {   // not even one block per row of replicas fits
+    (void)cudaGetLastError();
+    if (c->variant == 5) return cuda_fail(e, "ic_set_variant(5) was asked for, but the one-launch kernel does not fit this GPU partition");
+    c->coop_supported = false;                     // automatic selection: the per-phase kernels from now on
     return 1;
   }
   IC_CUDA(e);
@@ -506,7 +517,7 @@ static int launch_coop(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
 static bool resvec_ok(const ic_ctx* c) { return c->L >= RESV_MIN_L && c->L <= RESV_MAX_L; }
 template <int LAYG>
 static int launch_resvec(ic_ctx* c, int64_t nsweeps, int64_t* d_trace) {
-  static bool configured[64] = {};
+  static std::atomic<bool> configured[64] = {};
   if (c->device < 0 || c->device >= 64 || !configured[c->device]) {
     IC_CUDA(cudaFuncSetAttribute(k_resvec_sweeps<LAYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESV_SMEM_BYTES));
     if (c->device >= 0 && c->device < 64) configured[c->device] = true;
@@ -609,7 +620,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     int rc = c->layout == LAY_P2 ? launch_coop<2>(c, nsweeps, d_trace) : launch_coop<8>(c, nsweeps, d_trace);
     if (rc < 0) return rc;
     if (rc == IC_OK) { c->sweep += (uint64_t)nsweeps; return IC_OK; }
-    if (c->variant == 5) c->variant = 0;           // rc > 0: the cooperative launch does not fit; fall through to the phase kernels
+    // rc > 0 (automatic selection only): the cooperative launch does not fit; fall through to the phase kernels
   }
 
   PhaseArgs a;
@@ -684,6 +695,32 @@ extern "C" int ic_observables(ic_ctx* c, ic_obs* h_out) {
       q.chi_s = (mMs2 - mMs * mMs) / (Nd * T);
     }
   }
+  return IC_OK;
+}
+
+// Resume (lattice + global sweep counter + seed determine the future; the fp64 sums continue the averages).
+extern "C" int ic_restore(ic_ctx* c, int64_t sweep_count, const ic_obs* h_in) {
+  if (!c || !h_in) return IC_ERR_NULL;
+  if (sweep_count < 0 || (uint64_t)sweep_count >= (1ull << 31)) return IC_ERR_PARAM;
+  for (int r = 0; r < c->replicas; ++r) {
+    const ic_obs& q = h_in[r];
+    const double v[8] = {q.sumE, q.sumE2, q.sumM, q.sumM2, q.sumAbsM, q.sumMs, q.sumMs2, q.sumAbsMs};
+    if (q.nmeas < 0) return IC_ERR_PARAM;
+    for (double x : v) if (!std::isfinite(x)) return IC_ERR_PARAM;
+  }
+  IC_ENTER(c);
+  // the integers of the current lattices stay as they are (ic_set_state recomputed them); only nmeas and the sums change
+  IC_CUDA(cudaMemcpyAsync(c->h_obs, c->d_obs, (size_t)c->replicas * sizeof(ReplicaObs), cudaMemcpyDeviceToHost, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  for (int r = 0; r < c->replicas; ++r) {
+    ReplicaObs& o = c->h_obs[r];
+    const ic_obs& q = h_in[r];
+    o.nmeas = q.nmeas; o.sumE = q.sumE; o.sumE2 = q.sumE2; o.sumM = q.sumM; o.sumM2 = q.sumM2; o.sumAbsM = q.sumAbsM;
+    o.sumMs = q.sumMs; o.sumMs2 = q.sumMs2; o.sumAbsMs = q.sumAbsMs;
+  }
+  IC_CUDA(cudaMemcpyAsync(c->d_obs, c->h_obs, (size_t)c->replicas * sizeof(ReplicaObs), cudaMemcpyHostToDevice, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  c->sweep = (uint64_t)sweep_count;
   return IC_OK;
 }
 

@@ -33,12 +33,17 @@ constexpr int COOP_OFF_THR = 0;                                    // uint32 thr
 constexpr int COOP_OFF_DESC = COOP_OFF_THR + THR_STRIDE * 8;       // [2 sweep types] uint2 descriptors [8][28][16]
 constexpr int COOP_SMEM_BYTES = COOP_OFF_DESC + 2 * ST_DESC_SMEM;
 
-struct CoopScratch {            // one per replica, in the workspace; zeroed before every launch
+struct CoopScratch {            // one per replica, in the workspace; set up before every launch: acc = 0, arrived = COOP_BAR_BASE
   long long acc[2][5];          // per-sweep sums (dn2, dV, dJ, M, Ms of the updated sites), buffer = sweep parity
-  unsigned int arrived;         // barrier counter of the replica's blocks (monotonic within a launch)
+  unsigned int arrived;         // barrier counter of the replica's blocks: + gridDim.x per barrier, modulo 2^32
   unsigned int pad[11];
 };
 static_assert(sizeof(CoopScratch) == 128, "CoopScratch layout");
+// The counter grows by gridDim.x at each of the 2 nsweeps + 1 barriers of a launch and ic_sweep accepts up to 2^31 sweeps, so
+// it wraps in a long call (148 blocks: after 14.5 M sweeps).  The barrier therefore compares modulo 2^32 (a block is never
+// more than one barrier = gridDim.x < 2^31 counts away from the counter), and the counter STARTS one count below 2^32: every
+// launch, hence every test of this kernel, crosses the wrap at its first barrier.
+constexpr unsigned int COOP_BAR_BASE = 0xFFFFFFFFu;
 
 struct CoopArgs {
   void* lattice; const uint2* thr; const uint2* desc32; ReplicaObs* obs; CoopScratch* scratch;
@@ -60,7 +65,7 @@ __device__ __forceinline__ void coop_barrier(unsigned int* counter, unsigned int
   __syncthreads();                 // the block's writes happen before thread 0's release (causality order through the barrier)
   if (threadIdx.x == 0) {
     asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
-    while (ld_acquire_u32(counter) < target) { }
+    while ((int)(ld_acquire_u32(counter) - target) < 0) { }      // modulo 2^32: correct across the wrap of the counter
   }
   __syncthreads();
 }
@@ -278,7 +283,7 @@ __global__ void __launch_bounds__(COOP_THREADS, 1) k_coop_sweeps(const CoopArgs 
   ReplicaObs o;
   if (folder) o = A.obs[r];
   if (tid == nit) sweep_schedule(L, A.sweep0, A.key0, A.key1, s_par[0]);
-  unsigned int bar_target = 0;
+  unsigned int bar_target = COOP_BAR_BASE;
   __syncthreads();
 
   // sums of sweep q: block -> the replica's accumulator acc[q & 1] (service warp); accumulator -> integers -> fold (folder)

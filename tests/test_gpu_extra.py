@@ -20,7 +20,8 @@ def pkg():
 
 
 @pytest.mark.parametrize("L,bits,reps,K,nmaps", [(4, 8, 2, 3, 300), (16, 8, 3, 26, 200), (16, 2, 2, 60, 200), (64, 8, 3, 410, 120),
-                                                 (64, 2, 2, 820, 60), (256, 8, 2, 6554, 40), (1024, 8, 1, 100000, 6)])
+                                                 (64, 2, 2, 820, 60), (256, 8, 2, 6554, 40), (1024, 8, 1, 100000, 6),
+                                                 (256, 2, 2, 6554, 40), (1024, 2, 1, 100000, 6)])   # 2 bits, L >= 128: layout P2
 def test_map_sweeps_match_the_oracle(pkg, L, bits, reps, K, nmaps):
     """ic_sweep_maps: every map's candidates, survivors and pair updates equal the oracle's (mode 1), bit for bit: lattices,
     per-map integers, fp64 sums; sum S = Q after every map."""
@@ -61,7 +62,8 @@ def test_map_sweeps_argument_checks(pkg):
     sim.close()
 
 
-@pytest.mark.parametrize("L,bits,dens", [(4, 8, 0.5), (16, 8, 0.55), (16, 2, 0.3), (64, 8, 0.6), (64, 2, 0.45), (256, 8, 0.59), (2048, 8, 0.55)])
+@pytest.mark.parametrize("L,bits,dens", [(4, 8, 0.5), (16, 8, 0.55), (16, 2, 0.3), (64, 8, 0.6), (64, 2, 0.45), (256, 8, 0.59), (2048, 8, 0.55),
+                                         (256, 2, 0.59), (2048, 2, 0.55)])                            # 2 bits, L >= 128: layout P2
 def test_largest_cluster_matches_the_oracle(pkg, L, bits, dens):
     """ic_largest_cluster (union-find on the device) against the oracle's flood fill, near the site-percolation threshold
     (0.593) where clusters are large and ragged; all three charge selections; two replicas."""

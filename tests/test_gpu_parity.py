@@ -191,6 +191,45 @@ def test_call_splitting_and_reset(pkg):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("L,bits,bits2", [(8, 8, 8), (64, 8, 2), (256, 2, 8), (1024, 8, 8), (2048, 8, 2)])
+def test_resume_continues_the_same_trajectory(pkg, L, bits, bits2):
+    """SURVEY sec. 5 (checkpoint / resume): lattice + sweep counter + seed determine the future.  40 sweeps in one context ==
+    17 sweeps, save (ic_state, ic_sweep_count, ic_observables), a NEW context (other bits per site allowed), ic_set_state +
+    ic_restore, 23 sweeps: lattices, exact integers and the fp64 sums equal with ==, for every kernel family."""
+    seed, reps, Ts = 90 + L, 2, [0.8, 1.7]
+    N = L * L
+    nplus, nminus = N // 8, N // 16
+    n = (nplus - nminus) / N
+    codes = [ic_inputs.random_state(L, nplus, nminus, seed, r) for r in range(reps)]
+    a = pkg.Sim(L, n, 0.4, 1.0, 1.2, seed=seed, replicas=reps, bits_per_site=bits)
+    b = pkg.Sim(L, n, 0.4, 1.0, 1.2, seed=seed, replicas=reps, bits_per_site=bits)
+    for r in range(reps):
+        a.set_state(r, codes[r]); b.set_state(r, codes[r])
+    a.sweep(Ts, 40)
+    b.sweep(Ts, 17)
+    saved = ([b.state(r).copy() for r in range(reps)], b.sweep_count, b.observables())
+    b.close()
+    c = pkg.Sim(L, n, 0.4, 1.0, 1.2, seed=seed, replicas=reps, bits_per_site=bits2)
+    for r in range(reps):
+        c.set_state(r, saved[0][r])
+    for bad in (lambda: c.restore(-1, saved[2]), lambda: c.restore(1 << 31, saved[2]),
+                lambda: c.restore(17, [dict(saved[2][0], sumE=float("nan")), saved[2][1]]),
+                lambda: c.restore(17, [dict(saved[2][0], nmeas=-1), saved[2][1]])):
+        with pytest.raises(pkg.IcError):
+            bad()
+    assert c.sweep_count == 0
+    c.restore(saved[1], saved[2])
+    assert c.sweep_count == 17
+    c.sweep(Ts, 23)
+    assert c.sweep_count == a.sweep_count == 40
+    oa, oc = a.observables(), c.observables()
+    for r in range(reps):
+        assert np.array_equal(a.state(r), c.state(r)), r
+        assert oa[r] == oc[r], (r, oa[r], oc[r])
+        assert oa[r]["nmeas"] == 40
+    a.close(); c.close()
+
+
 def test_frozen_and_degenerate_lattices(pkg):
     L = 32
     # n = +-1: every pair has q = +-2, nothing can move; E = N (Delta + 2V) exactly (SURVEY P9)
@@ -316,6 +355,8 @@ def test_config_c5_full_size_sampled(pkg, bits):
     sim = pkg.Sim(L, c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=bits)
     code = sim.state(0).copy()
     assert int(S_OF[code].sum()) == sim.Q == c["nplus"]
+    kinds = {("FAR",) if k[0] == 0 else ("NEAR", k[1]) for k in (sim.schedule(s) for s in range(5))}
+    assert kinds == {("FAR",), ("NEAR", 0), ("NEAR", 1)}, kinds     # the compared sweeps run all three kernels: FAR, NEAR-H, NEAR-V
     sim.sweep(c["T"], 5)
     if "C5" not in _ORACLE_RUNS:
         lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
