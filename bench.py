@@ -197,6 +197,8 @@ def main():
     ap.add_argument("--sweeps-per-step", type=int, default=0, help="0 = the sweeps of the config's whole run (C5: 100)")
     ap.add_argument("--bits", type=int, default=0, help="override bits per site (8 or 2)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = automatic)")
+    ap.add_argument("--replicas", type=int, default=0, help="override the number of lattice copies per GPU (temperatures repeat cyclically): "
+                    "with >= 4 x the SM count a small-lattice config shows its saturated rate instead of its latency-bound one")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the timed CPU-oracle sample")
     ap.add_argument("--no-e2e", action="store_true")
@@ -204,6 +206,8 @@ def main():
     cfg = dict(ic_inputs.CONFIGS[args.config])
     if args.bits:
         cfg["bits"] = args.bits
+    if args.replicas > 0:
+        cfg["T"] = [cfg["T"][i % len(cfg["T"])] for i in range(args.replicas)]
     if args.sweeps_per_step <= 0:
         args.sweeps_per_step = int(cfg["sweeps"])
     if args.impl == "reference":
@@ -294,6 +298,29 @@ def main():
                "h2d_bytes_per_step": reps * N + 8 * reps, "d2h_bytes_per_step": reps * N + 128 * reps, "steps": e2e_steps,
                "path": "ic_set_state(pinned host) -> ic_sweep -> ic_state(pinned host) + ic_observables"}
 
+    # ---- the same with the host lattices at 2 bits per site (ic_set_state_packed / ic_state_packed): a quarter of the PCIe bytes
+    e2e_packed = None
+    if not args.no_e2e:
+        del host_in, host_out
+        pk_in = torch.empty((reps, N // 4), dtype=torch.uint8).pin_memory()
+        pk_out = torch.empty((reps, N // 4), dtype=torch.uint8).pin_memory()
+        for r in range(reps):
+            sim.state_packed(r, out=pk_in[r])
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            for r in range(reps):
+                sim.set_state_packed(r, pk_in[r])     # H2D of the step's input lattice, 2 bits per site (eq. 2 checked on the device)
+            sim.sweep(Ts, S)
+            for r in range(reps):
+                sim.state_packed(r, out=pk_out[r])    # D2H of the result lattice, 2 bits per site
+            o = sim.observables()
+        barrier()
+        dt = shard.max_over_ranks(time.perf_counter() - t0)
+        e2e_packed = {"value": world * pairs_per_step * e2e_steps / (dt * 1e9), "unit": UNIT,
+                      "h2d_bytes_per_step": reps * N // 4 + 8 * reps, "d2h_bytes_per_step": reps * N // 4 + 128 * reps, "steps": e2e_steps,
+                      "path": "ic_set_state_packed(pinned host, 2 bits/site) -> ic_sweep -> ic_state_packed(pinned host) + ic_observables"}
+
     # ---- roofline of the dominant kernel (one phase launch = N/4 pair updates per replica) ----------------------------------
     peak, peak_src = measured_peaks()
     phase_launches = 2 * S * args.steps
@@ -334,6 +361,7 @@ def main():
         }
         if e2e:
             out["e2e"] = e2e
+            out["e2e_packed"] = e2e_packed
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
             Ls = min(L, 8192)

@@ -110,6 +110,15 @@ int ic_reset_observables(ic_ctx* ctx);            /* zeroes nmeas and the fp64 s
 int ic_observables(ic_ctx* ctx, ic_obs* h_out);   /* h_out[replicas], HOST; synchronises the stream    */
 int ic_state(ic_ctx* ctx, int replica, int8_t* h_codes_out); /* L*L public codes, HOST; synchronises   */
 
+/* The same two calls with the lattice at 2 bits per site on the host side too (a site has four states;
+ * BASELINE north_star: "lattice packed at 2 bits or 1 byte per site"): h_words[L*L/16] (HOST), word i holds the sites
+ * 16 i .. 16 i + 15 of the row-major lattice, the public code of site k of the word in bits 2k and 2k+1.  A quarter of the
+ * bytes cross PCIe; checking (sum S == Q -- every 2-bit pattern is a valid code) and conversion to and from the context's
+ * layout run on the device.  Any bits_per_site.  Both synchronise the stream.  A rejected lattice (IC_ERR_CHARGE) leaves
+ * the replica untouched.                                                                                                  */
+int ic_set_state_packed(ic_ctx* ctx, int replica, const uint32_t* h_words);
+int ic_state_packed(ic_ctx* ctx, int replica, uint32_t* h_words_out);
+
 /* Resume.  The lattices, the global sweep counter and the seed determine every later pair update (the random stream is
  * keyed by (seed, replica, sweep, slot)); nmeas and the fp64 sums carry the averages of PAPER.md:49-53 across the break.
  * To save a run: ic_state of every replica, ic_sweep_count, ic_observables.  To continue it: ic_create with the same L, n,

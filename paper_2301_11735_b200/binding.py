@@ -36,6 +36,8 @@ EXPORTS = {
     "ic_reset_observables": (C.c_int, [C.c_void_p]),
     "ic_observables": (C.c_int, [C.c_void_p, C.POINTER(ic_obs)]),
     "ic_state": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "ic_set_state_packed": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "ic_state_packed": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "ic_restore": (C.c_int, [C.c_void_p, C.c_int64, C.POINTER(ic_obs)]),
     "ic_debug_recompute": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]),
     "ic_thresholds": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(C.c_uint32)]),
@@ -199,6 +201,24 @@ class Sim:
         out = (ic_obs * self.replicas)()
         _check(lib.ic_observables(self.h, out), "ic_observables")
         return [{f: getattr(o, f) for f, _ in ic_obs._fields_} for o in out]
+
+    def set_state_packed(self, replica, words):
+        """words: numpy uint32 [L*L/16] (or a pinned torch CPU tensor of that many bytes x 4): 16 public codes per word."""
+        if hasattr(words, "data_ptr"):
+            assert words.device.type == "cpu" and words.is_contiguous() and words.numel() * words.element_size() == self.N // 4
+            ptr = words.data_ptr()
+        else:
+            words = np.ascontiguousarray(words, dtype=np.uint32)
+            assert words.size == self.N // 16
+            ptr = words.ctypes.data
+        _check(lib.ic_set_state_packed(self.h, int(replica), C.c_void_p(ptr)), "ic_set_state_packed")
+
+    def state_packed(self, replica=0, out=None):
+        if out is None:
+            out = np.empty(self.N // 16, dtype=np.uint32)
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        _check(lib.ic_state_packed(self.h, int(replica), C.c_void_p(ptr)), "ic_state_packed")
+        return out
 
     def restore(self, sweep_count, observables):
         """ic_restore: continue a saved run -- `observables` is what observables() returned when the run was saved."""

@@ -33,7 +33,7 @@ struct ic_ctx {
   cudaStream_t stream;
   // device (inside the caller's workspace)
   char* lattice; long long lat_stride;
-  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; CoopScratch* d_coop; unsigned int* d_task_ctr; int8_t* d_stage;
+  uint2* d_thr; uint2* d_desc; uint2* d_desc32; ReplicaObs* d_obs; long long* d_scratch8; CoopScratch* d_coop; unsigned int* d_task_ctr; int8_t* d_stage; uint32_t* d_stage2;
   // host (pinned)
   uint2* h_thr; ReplicaObs* h_obs;
   cudaEvent_t thr_copied;
@@ -84,6 +84,7 @@ extern "C" size_t ic_workspace_bytes(int L, int replicas, int bits) {
   b += align256((size_t)replicas * sizeof(CoopScratch));           // per-sweep sums and barrier counters of the one-launch kernel
   b += align256((size_t)replicas * TASK_CTR_STRIDE * 4);           // task counters of the staged kernels
   b += align256((size_t)L * L);                                    // staging of one lattice in public byte codes
+  b += align256((size_t)L * L / 4);                                // ... and in packed public codes (ic_set_state_packed / ic_state_packed)
   return b;
 }
 
@@ -248,6 +249,7 @@ static int recompute_into_scratch(ic_ctx* c, int replica) {
 // Uploads public byte codes (host) into the replica's lattice and refreshes its exact integers.  With `validate` the
 // codes are first checked on the device in the staging buffer (every code in 0..3, sum S == Q: eq. 2); a
 // rejected lattice leaves the replica untouched.
+static int install_staged_codes(ic_ctx* c, int replica);
 static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, bool validate) {
   char* lat = c->lattice + (long long)replica * c->lat_stride;
   const long long n16 = c->N / 16;
@@ -263,6 +265,13 @@ static int upload_state(ic_ctx* c, int replica, const int8_t* h_codes, bool vali
     IC_CUDA(cudaStreamSynchronize(c->stream));
     if (h[0] != 0 || h[1] != c->Q) return IC_ERR_CHARGE;
   }
+  return install_staged_codes(c, replica);
+}
+// the lattice in public byte codes in the staging buffer -> the replica's layout; recomputes its exact integers
+static int install_staged_codes(ic_ctx* c, int replica) {
+  char* lat = c->lattice + (long long)replica * c->lat_stride;
+  const long long n16 = c->N / 16;
+  const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
   if (c->layout == LAY_ROW8) IC_CUDA(cudaMemcpyAsync(lat, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToDevice, c->stream));
   else {
     if (c->layout == LAY_ROW2) k_pack2<<<blocks, 256, 0, c->stream>>>(c->d_stage, (uint32_t*)lat, n16);
@@ -306,7 +315,8 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   c->d_scratch8 = (long long*)p; p += 256;
   c->d_coop = (CoopScratch*)p; p += align256((size_t)replicas * sizeof(CoopScratch));
   c->d_task_ctr = (unsigned int*)p; p += align256((size_t)replicas * TASK_CTR_STRIDE * 4);
-  c->d_stage = (int8_t*)p;
+  c->d_stage = (int8_t*)p; p += align256((size_t)c->N);
+  c->d_stage2 = (uint32_t*)p;
   c->h_thr = nullptr; c->h_obs = nullptr; c->thr_copied = nullptr;
 
   auto fail = [&](int rc) { ic_destroy(c); return rc; };
@@ -401,6 +411,65 @@ extern "C" int ic_state(ic_ctx* c, int replica, int8_t* h_out) {
     IC_CUDA(cudaGetLastError());
     IC_CUDA(cudaMemcpyAsync(h_out, c->d_stage, (size_t)c->N, cudaMemcpyDeviceToHost, c->stream));
   }
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  return IC_OK;
+}
+
+// ---- lattices at 2 bits per site over PCIe (a site has four states) -----------------------------------------
+// The packed public format is layout ROW2: word i holds the sites 16 i .. 16 i + 15 of the row-major lattice, site k of the
+// word in bits 2k, 2k+1.  A quarter of the bytes of ic_set_state / ic_state cross the bus; the conversions run on the device.
+extern "C" int ic_set_state_packed(ic_ctx* c, int replica, const uint32_t* h_words) {
+  if (!c || !h_words) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  IC_ENTER(c);
+  const long long n16 = c->N / 16;
+  const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
+  IC_CUDA(cudaMemcpyAsync(c->d_stage2, h_words, (size_t)c->N / 4, cudaMemcpyHostToDevice, c->stream));
+  IC_CUDA(cudaMemsetAsync(c->d_scratch8, 0, 64, c->stream));
+  k_charge_of_packed<<<blocks, 256, 0, c->stream>>>(c->d_stage2, n16, c->d_scratch8);
+  c->launches++;
+  IC_CUDA(cudaGetLastError());
+  long long h[2];
+  IC_CUDA(cudaMemcpyAsync(h, c->d_scratch8, 16, cudaMemcpyDeviceToHost, c->stream));
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  if (h[1] != c->Q) return IC_ERR_CHARGE;                              // the replica is untouched
+  if (c->layout == LAY_ROW2) {                                         // the packed format is the layout
+    IC_CUDA(cudaMemcpyAsync(c->lattice + (long long)replica * c->lat_stride, c->d_stage2, (size_t)c->N / 4, cudaMemcpyDeviceToDevice, c->stream));
+    int rc = recompute_into_scratch(c, replica);
+    if (rc != IC_OK) return rc;
+    k_store_ints<<<1, 1, 0, c->stream>>>(&c->d_obs[replica], c->d_scratch8);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+  } else {
+    k_unpack2<<<blocks, 256, 0, c->stream>>>(c->d_stage2, c->d_stage, n16);
+    c->launches++;
+    IC_CUDA(cudaGetLastError());
+    int rc = install_staged_codes(c, replica);
+    if (rc != IC_OK) return rc;
+  }
+  IC_CUDA(cudaStreamSynchronize(c->stream));
+  return IC_OK;
+}
+
+extern "C" int ic_state_packed(ic_ctx* c, int replica, uint32_t* h_out) {
+  if (!c || !h_out) return IC_ERR_NULL;
+  if (replica < 0 || replica >= c->replicas) return IC_ERR_SIZE;
+  IC_ENTER(c);
+  const char* lat = c->lattice + (long long)replica * c->lat_stride;
+  const long long n16 = c->N / 16;
+  const int blocks = (int)std::min<long long>((n16 + 255) / 256, (long long)c->sm_count * 16);
+  const void* src = c->d_stage2;
+  if (c->layout == LAY_ROW2) src = lat;
+  else {
+    const int8_t* codes = c->d_stage;
+    if (c->layout == LAY_ROW8) codes = (const int8_t*)lat;
+    else if (c->layout == LAY_P2) k_p2_to_codes<<<std::max(1, blocks / 4), 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
+    else k_p16_to_codes<<<blocks, 256, 0, c->stream>>>((const uint8_t*)lat, c->d_stage, c->logL);
+    k_pack2<<<blocks, 256, 0, c->stream>>>(codes, c->d_stage2, n16);
+    c->launches += c->layout == LAY_ROW8 ? 1 : 2;
+    IC_CUDA(cudaGetLastError());
+  }
+  IC_CUDA(cudaMemcpyAsync(h_out, src, (size_t)c->N / 4, cudaMemcpyDeviceToHost, c->stream));
   IC_CUDA(cudaStreamSynchronize(c->stream));
   return IC_OK;
 }

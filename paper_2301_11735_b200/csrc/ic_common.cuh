@@ -41,7 +41,8 @@ IC_HD u32x4 philox4x32(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // Schedule and stage-1 streams: the default ten rounds.  Update stream (one block per four pair updates, the hot path):
 // Philox4x32-7, the seven-round member of the family that Salmon et al. report as the fewest rounds passing BigCrush
 // (SURVEY 8(d) "RNG ladder", G5).
-// Compile-time switch (the oracle's twin is orc_set_update_rounds): build with -DIC_PHILOX_UPDATE_ROUNDS=10 for the default
+// Compile-time switch (G5 names the test that compares the sampled ensembles at 7 and 10 rounds): build with
+// -DIC_PHILOX_UPDATE_ROUNDS=10 for the default
 // member of the family; every kernel, the staged kernels' precomputed round keys included, follows this constant.
 #ifndef IC_PHILOX_UPDATE_ROUNDS
 #define IC_PHILOX_UPDATE_ROUNDS 7

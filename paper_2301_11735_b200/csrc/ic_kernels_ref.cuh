@@ -237,4 +237,16 @@ __global__ void k_unpack2(const uint32_t* words, int8_t* codes, long long n16) {
   }
 }
 
+// Sum S of a lattice in packed public codes (ic_set_state_packed): every 2-bit pattern is a valid code, so eq. (2)
+// is the only thing to check.  code bit1 = charge, bit0 = negative.  out2[1] += sum S.
+__global__ void __launch_bounds__(256) k_charge_of_packed(const uint32_t* words, long long n16, long long* out2) {
+  long long q = 0;
+  for (long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x; wi < n16; wi += (long long)gridDim.x * blockDim.x) {
+    const uint32_t wd = words[wi], ch = (wd >> 1) & 0x55555555u;
+    q += __popc(ch) - 2 * __popc(ch & wd);
+  }
+  for (int o = 16; o > 0; o >>= 1) q += __shfl_down_sync(0xFFFFFFFFu, q, o);
+  if ((threadIdx.x & 31) == 0 && q) atomicAdd((unsigned long long*)&out2[1], (unsigned long long)q);
+}
+
 }  // namespace ic

@@ -230,6 +230,47 @@ def test_resume_continues_the_same_trajectory(pkg, L, bits, bits2):
     a.close(); c.close()
 
 
+def _pack_codes(code):
+    """Public packing of ic.h: word i = sites 16 i .. 16 i + 15 of the row-major lattice, site k in bits 2k, 2k+1 (plain numpy)."""
+    c = np.asarray(code, dtype=np.uint32).reshape(-1, 16)
+    return (c << (2 * np.arange(16, dtype=np.uint32))).sum(axis=1, dtype=np.uint64).astype(np.uint32)
+
+
+@pytest.mark.parametrize("L,bits", [(4, 8), (4, 2), (32, 8), (64, 2), (64, 8), (256, 2), (1024, 8), (2048, 8), (2048, 2)])
+def test_packed_state_calls(pkg, L, bits):
+    """ic_set_state_packed / ic_state_packed (2 bits per site on the host side) against the byte calls in every
+    layout (ROW8, ROW2, P16, P2): the same lattice, the same integers, the same trajectory afterwards; a lattice with the
+    wrong charge is refused and leaves the replica as it was."""
+    N = L * L
+    nplus, nminus = N // 4, N // 8
+    n = (nplus - nminus) / N
+    code = ic_inputs.random_state(L, nplus, nminus, 700 + L, 0)
+    words = _pack_codes(code)
+    a = pkg.Sim(L, n, 0.3, 1.0, 0.8, seed=9, replicas=2, bits_per_site=bits)
+    b = pkg.Sim(L, n, 0.3, 1.0, 0.8, seed=9, replicas=2, bits_per_site=bits)
+    before = b.state(1).copy()
+    a.set_state(1, code); b.set_state_packed(1, words)
+    assert np.array_equal(b.state(1), code) and np.array_equal(b.state_packed(1), words)
+    assert np.array_equal(a.state_packed(1), words)
+    assert np.array_equal(b.state(0), a.state(0))                        # the other replica is untouched
+    assert list(b.debug_recompute(1)) == list(a.debug_recompute(1))
+    oa, ob = a.observables(), b.observables()
+    assert all(oa[1][k] == ob[1][k] for k in ("n2", "bV", "bJ", "M", "Ms", "Q"))
+    bad = code.copy().reshape(-1)
+    bad[np.flatnonzero(bad < 2)[0]] = 2                                  # one charge too many
+    with pytest.raises(pkg.IcError) as e:
+        b.set_state_packed(0, _pack_codes(bad))
+    assert e.value.code == pkg.IC_ERR_CHARGE
+    assert np.array_equal(b.state(0), a.state(0)) and np.array_equal(b.state(1), code)
+    a.sweep([0.9, 1.4], 6); b.sweep([0.9, 1.4], 6)
+    for r in range(2):
+        assert np.array_equal(a.state(r), b.state(r))
+        assert np.array_equal(_pack_codes(a.state(r)), b.state_packed(r))
+    assert a.observables() == b.observables()
+    assert before.shape == (L, L)
+    a.close(); b.close()
+
+
 def test_frozen_and_degenerate_lattices(pkg):
     L = 32
     # n = +-1: every pair has q = +-2, nothing can move; E = N (Delta + 2V) exactly (SURVEY P9)
