@@ -216,6 +216,11 @@ int ic_largest_cluster_static(const int8_t* d_codes, int L, int which, int64_t* 
  * lattices and observables.                                                                           */
 int ic_set_variant(ic_ctx* ctx, int variant);
 
+/* The kernel family the last ic_sweep / ic_sweep_trace call of this context ran, in the numbering of ic_set_variant (1..6);
+ * 0 before the first sweep, -1 if ctx is NULL.  With automatic selection this is how a caller (and the tests) see which
+ * kernels did the work, e.g. that a cooperative launch that did not fit the GPU partition fell back to the phase kernels.  */
+int ic_kernel_family(const ic_ctx* ctx);
+
 /* Upper bound on the thread blocks per replica of the persistent kernels (variants 2, 3, 5); 0 = automatic (one block per
  * SM divided among the replicas).  Results do not depend on it: the tests run the kernels at several bounds (1, 2, 3, ...)
  * so that every block walks many tasks and ring laps and the task-to-block assignment changes -- the race check this

@@ -53,6 +53,7 @@ EXPORTS = {
     "ic_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
     "ic_set_max_blocks": (C.c_int, [C.c_void_p, C.c_int]),
     "ic_launch_count": (C.c_int64, [C.c_void_p]),
+    "ic_kernel_family": (C.c_int, [C.c_void_p]),
     "ic_destroy": (C.c_int, [C.c_void_p]),
     "ic_strerror": (C.c_char_p, [C.c_int]),
 }
@@ -264,6 +265,11 @@ class Sim:
     @property
     def Q(self):
         return int(lib.ic_charge(self.h))
+
+    @property
+    def kernel_family(self):
+        """Variant number (1..6, see ic_set_variant) of the kernels the last sweep call ran; 0 before the first sweep."""
+        return int(lib.ic_kernel_family(self.h))
 
     @property
     def launch_count(self):

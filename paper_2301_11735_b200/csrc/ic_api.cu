@@ -42,6 +42,7 @@ struct ic_ctx {
   int sm_count, device;
   bool coop_supported;
   int max_blocks;            // ic_set_max_blocks: 0 = automatic
+  int last_family;           // ic_kernel_family: the variant number of the kernels the last sweep call ran (0: none yet)
 };
 static long long blocks_cap(const ic_ctx* c, long long automatic) {
   return c->max_blocks > 0 ? std::min<long long>(automatic, c->max_blocks) : automatic;
@@ -300,7 +301,7 @@ extern "C" int ic_create(ic_ctx** out, int L, double n, double delta, double V, 
   ic_ctx* c = new (std::nothrow) ic_ctx();
   if (!c) return IC_ERR_NULL;
   c->L = L; c->logL = 0; while ((1 << c->logL) < L) c->logL++;
-  c->replicas = replicas; c->bits = bits; c->variant = 0; c->max_blocks = 0;
+  c->replicas = replicas; c->bits = bits; c->variant = 0; c->max_blocks = 0; c->last_family = 0;
   c->layout = bits == 2 ? (L >= 128 ? LAY_P2 : LAY_ROW2) : (L >= 64 ? LAY_P16 : LAY_ROW8);
   c->N = (long long)L * L; c->Q = std::llround(n * (double)c->N);
   c->n = n; c->delta = delta; c->V = V; c->J = J; c->seed = seed; c->sweep = 0;
@@ -666,7 +667,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     int rc = c->layout == LAY_ROW8 ? launch_resvec<LAY_ROW8>(c, nsweeps, d_trace)
              : c->layout == LAY_ROW2 ? launch_resvec<LAY_ROW2>(c, nsweeps, d_trace) : launch_resvec<LAY_P16>(c, nsweeps, d_trace);
     if (rc != IC_OK) return rc;
-    c->sweep += (uint64_t)nsweeps;
+    c->sweep += (uint64_t)nsweeps; c->last_family = 6;
     return IC_OK;
   }
   if (c->L <= RES_MAX_L && (c->variant == 0 || c->variant == 4)) {
@@ -680,7 +681,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
     else k_resident_sweeps<LAY_P16><<<c->replicas, rthreads, 0, c->stream>>>(ra);
     c->launches++;
     IC_CUDA(cudaGetLastError());
-    c->sweep += (uint64_t)nsweeps;
+    c->sweep += (uint64_t)nsweeps; c->last_family = 4;
     return IC_OK;
   }
 
@@ -688,7 +689,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
   if (coop_ok(c) && (c->variant == 0 || c->variant == 5)) {
     int rc = c->layout == LAY_P2 ? launch_coop<2>(c, nsweeps, d_trace) : launch_coop<8>(c, nsweeps, d_trace);
     if (rc < 0) return rc;
-    if (rc == IC_OK) { c->sweep += (uint64_t)nsweeps; return IC_OK; }
+    if (rc == IC_OK) { c->sweep += (uint64_t)nsweeps; c->last_family = 5; return IC_OK; }
     // rc > 0 (automatic selection only): the cooperative launch does not fit; fall through to the phase kernels
   }
 
@@ -706,6 +707,7 @@ static int sweep_impl(ic_ctx* c, const double* h_T, int64_t nsweeps, int64_t* d_
       const bool staged = staged_ok(c) && (c->variant == 3 || c->variant == 0);
       const bool tiled = tiled_ok(c) && (c->variant == 0 || c->variant == 2);
       absolute = staged;     // the staged kernels report M, Ms of the updated sites instead of their changes
+      c->last_family = staged ? 3 : tiled ? 2 : 1;
       int rc = staged ? launch_phase_staged(c, a) : tiled ? launch_phase_p16(c, a) : launch_phase_ref(c, a);
       if (rc != IC_OK) return rc;
     }
@@ -994,6 +996,7 @@ extern "C" int ic_schedule(ic_ctx* c, uint64_t sweep, int32_t* out4) {
 
 extern "C" int64_t ic_sweep_count(const ic_ctx* c) { return c ? (int64_t)c->sweep : -1; }
 extern "C" int64_t ic_charge(const ic_ctx* c) { return c ? (int64_t)c->Q : 0; }
+extern "C" int ic_kernel_family(const ic_ctx* c) { return c ? c->last_family : -1; }
 extern "C" int64_t ic_launch_count(const ic_ctx* c) { return c ? (int64_t)c->launches : -1; }
 
 extern "C" int ic_set_variant(ic_ctx* c, int variant) {

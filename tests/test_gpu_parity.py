@@ -271,6 +271,21 @@ def test_packed_state_calls(pkg, L, bits):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("L,bits,family", [(8, 8, 4), (8, 2, 4), (16, 8, 6), (64, 2, 6), (128, 8, 5), (1024, 2, 5), (2048, 8, 3), (2048, 2, 3)])
+def test_automatic_selection_runs_the_documented_kernel_family(pkg, L, bits, family):
+    """ic_kernel_family: with automatic selection every lattice size runs the family ic.h and DESIGN.md name for it (no silent
+    fall-back to the one-thread-per-pair kernels), and an explicit variant is reported as such."""
+    sim = pkg.Sim(L, 0.1, 0.2, 1.0, 1.0, seed=3, bits_per_site=bits)
+    assert sim.kernel_family == 0
+    sim.sweep(1.0, 2)
+    assert sim.kernel_family == family
+    sim.set_variant(1); sim.sweep(1.0, 1)
+    assert sim.kernel_family == 1
+    sim.set_variant(0); sim.sweep(1.0, 1)
+    assert sim.kernel_family == family
+    sim.close()
+
+
 def test_frozen_and_degenerate_lattices(pkg):
     L = 32
     # n = +-1: every pair has q = +-2, nothing can move; E = N (Delta + 2V) exactly (SURVEY P9)
@@ -399,6 +414,7 @@ def test_config_c5_full_size_sampled(pkg, bits):
     kinds = {("FAR",) if k[0] == 0 else ("NEAR", k[1]) for k in (sim.schedule(s) for s in range(5))}
     assert kinds == {("FAR",), ("NEAR", 0), ("NEAR", 1)}, kinds     # the compared sweeps run all three kernels: FAR, NEAR-H, NEAR-V
     sim.sweep(c["T"], 5)
+    assert sim.kernel_family == 3                                    # the TMA-staged kernels bench.py times
     if "C5" not in _ORACLE_RUNS:
         lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
         lat.sweep_s1(c["T"][0], 5, threads=NCPU)
