@@ -434,6 +434,28 @@ def test_config_c5_full_size_sampled(pkg, bits):
     sim.close()
 
 
+@pytest.mark.skipif(os.environ.get("IC_LONG_TESTS") != "1", reason="whole-run comparison: about 3 minutes of oracle time; set IC_LONG_TESTS=1")
+def test_config_c5_whole_run_against_the_oracle(pkg):
+    """BASELINE config 5 for its WHOLE run (100 sweeps at L=16384, what one bench.py step executes), both state widths against the
+    multi-threaded oracle: lattice, exact integers and every fp64 sum equal.  Opt-in (IC_LONG_TESTS=1); the default suite
+    compares the first 5 sweeps (test_config_c5_full_size_sampled)."""
+    c = ic_inputs.CONFIGS["C5"]
+    sims = [pkg.Sim(c["L"], c["n"], c["delta"], c["V"], c["J"], seed=c["seed"], bits_per_site=b) for b in (8, 2)]
+    code = sims[0].state(0).copy()
+    for sim in sims:
+        sim.sweep(c["T"], c["sweeps"])
+        assert sim.kernel_family == 3
+    lat = oracle.Lattice(code, c["delta"], c["V"], c["J"], c["seed"])
+    lat.sweep_s1(c["T"][0], c["sweeps"], threads=NCPU)
+    ref = lat.observables(c["T"][0])
+    for sim in sims:
+        assert np.array_equal(sim.state(0), lat.code)
+        o = sim.observables()[0]
+        for k in ("nmeas", "n2", "bV", "bJ", "M", "Ms", "Q", "sumE", "sumE2", "sumM", "sumM2", "sumAbsM", "sumMs", "sumMs2", "sumAbsMs"):
+            assert o[k] == ref[k], (k, o[k], ref[k])
+        sim.close()
+
+
 def test_one_launch_kernel_with_more_replicas_than_sms(pkg):
     """More lattice copies than SMs at L = 128 (2 bits/site): every row of blocks of the one-launch kernel runs several
     replicas one after the other.  Three replicas against the oracle, all against eq. (2) and the recount."""
